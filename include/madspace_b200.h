@@ -1,0 +1,183 @@
+/*
+ * madspace_b200.h -- C ABI of the B200-native MadSpace phase-space hot path (arXiv 2602.06895).
+ *
+ * The library maps uniforms r in (0,1)^d to phase-space points x = G(r) with density g and
+ * returns the Monte Carlo weight 1/g [* f] (Eq. 1-5; forward Jacobian = 1/g,
+ * PAPER.md:112, Eq. 12).  Conventions follow the paper's own C interface style (UMAMI,
+ * PAPER.md:656-677): C-callable functions with fixed signatures, batched over events,
+ * device-resident pointers with a defined layout, no host<->device copies inside a call.
+ *
+ * COMMON CONVENTIONS
+ *  - Every pointer named d_* is a DEVICE pointer owned by the caller (torch tensors); h_* is a HOST
+ *    pointer.  The library allocates nothing, keeps no global state (except the last CUDA error
+ *    code) and never synchronises: each call validates its arguments on the host, enqueues its
+ *    kernel(s) on `stream` (a cudaStream_t passed as void*) and returns.
+ *  - Layout: structure of arrays, fp64.  A "row" is N consecutive doubles; a[row*ld + e] is the
+ *    value of event e, ld >= N the row stride in elements.  Base pointers must be 16-byte aligned.
+ *    Momentum rows: row = 4*particle + mu with mu = (E,px,py,pz) (Eq. 77 component
+ *    order); particles 0,1 are the incoming partons a,b, particles 2..n+1 the outgoing p_1..p_n
+ *    of Eq. 53.  A momentum block therefore has 4*(n+2) rows.
+ *  - Random numbers: Philox4x32-10, counter = (event_lo, event_hi, j>>1, stream), key = seed, where
+ *    event = rng.event_offset + e is the GLOBAL event index and j the uniform's dimension index;
+ *    uniform j takes output words (0,1) if j is even, (2,3) if odd: W = w_a<<32 | w_b,
+ *    u = (2*(W>>12)+1) * 2^-53, in the open interval (0,1) (readings R-1..R-3).
+ *    Wherever a uniform-row pointer may be NULL, NULL means "draw the uniforms in-kernel".
+ *  - Return value: MS_OK, or a negative code detected on the host BEFORE any launch (nothing was
+ *    enqueued), or MS_ECUDA when a launch failed (raw cudaError_t: ms_last_cuda_error()).
+ *  - Per-event failures (Newton cap hit, non-finite weight) do not fail the call: the event gets
+ *    weight 0 and, if d_fail != NULL, *d_fail (a device uint32 the caller zeroed) is incremented.
+ *  - n = number of outgoing particles, 2 <= n <= MS_MAX_N (k = n-2 <= 7: Table 1).
+ */
+#ifndef MADSPACE_B200_H
+#define MADSPACE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MS_MAX_N 9
+#define MS_MAX_DIMS 32      /* VEGAS grid dimensions */
+#define MS_MAX_BINS 1024    /* VEGAS bins per dimension; d*(n_bins+1)*16 B must fit 200 KB of shared memory */
+
+enum {
+    MS_OK = 0,
+    MS_EINVAL = -1,   /* null / misaligned pointer, N <= 0, n out of range, ld < N, bad flag */
+    MS_EGRID = -2,    /* reported by ms_check_grid: edges not strictly increasing, x_0 != 0 or x_nb != 1 */
+    MS_EKIN = -3,     /* sum of masses >= sqrt_s, tau_min outside (0,1), sqrt_s <= 0 with no per-event array */
+    MS_ECUDA = -4     /* kernel launch failed */
+};
+
+/* Counter-based RNG coordinates, passed by value (reading R-2). */
+typedef struct ms_rng {
+    uint64_t seed;          /* Philox key */
+    uint32_t stream;        /* 0: phase-space uniforms, 1: unweighting uniform */
+    uint32_t reserved;      /* must be 0 */
+    uint64_t event_offset;  /* global index of event 0 of this call */
+} ms_rng;
+
+const char* ms_version(void);
+int ms_last_cuda_error(void);
+
+/* Host-side validation of a VEGAS edge table h_edges[d][n_bins+1] (reading V-1):
+ * MS_OK, or MS_EGRID if any row is not 0 = x_0 < x_1 < ... < x_nb = 1, MS_EINVAL on bad sizes. */
+int ms_check_grid(int d, int n_bins, const double* h_edges);
+
+/* ms_vegas_map -- frozen VEGAS grid map (PAPER.md:603 "classic VEGAS", :746 grids adapted then
+ * frozen; the paper prints no equations: Lepage's piecewise-linear map, readings V-1..V-3).
+ *   direction 0 (forward):  t = r*n_bins, j = min(floor t, n_bins-1), x = x_j + (t-j)(x_{j+1}-x_j),
+ *       clamped into [2^-53, 1-2^-53]; d_jac[e] = prod_dims n_bins (x_{j+1}-x_j).
+ *       d_in = r rows [d][ld], or NULL -> Philox uniforms j = 0..d-1 of stream rng.stream.
+ *   direction 1 (inverse):  j = bin with x_j <= x < x_{j+1} (per-lane binary search over the
+ *       shared-memory edge table), r = (j + (x-x_j)/(x_{j+1}-x_j))/n_bins; d_jac[e] = 1/prod(...).
+ *       d_in = x rows (must not be NULL).
+ * d_edges: device table [d][n_bins+1], validated by the caller with ms_check_grid.
+ * d_out: [d][ld].  d_jac: [N] or NULL.  d_in and d_out may alias. */
+int ms_vegas_map(int64_t N, int d, int n_bins, const double* d_edges, int direction,
+                 const double* d_in, ms_rng rng, double* d_out, double* d_jac, int64_t ld, void* stream);
+
+/* ms_rambo_massless -- exact flat massless n-body phase space, RamboOnDiet (PAPER.md:405-474,
+ * Eq. 52-63): intermediate masses M_i = u_i M_{i-1} with u_i solving Eq. 62 (Newton, reading
+ * M-3), then n-1 two-body decays (Eq. 54-55, angles Eq. 25).  Weight is flat: d_w[e] = Phi_n(sqrt_s)
+ * of Eq. 81 (incl. (2 pi)^(4-3n)).
+ *   sqrt_s > 0: fixed CM energy; sqrt_s <= 0: per-event energies d_sqrt_s[N] (must be non-NULL).
+ *   d_x: [3n-4][ld] uniforms (rows 0..n-3 -> mass steps i=2..n-1; then (cos theta, phi) pairs per
+ *        decay, reading D-1), or NULL -> Philox j = 0..3n-5.
+ *   d_p: [4(n+2)][ld] out, frame = CM frame of Q_1; incoming rows = (sqrt_s/2)(1,0,0,+-1).
+ *   d_w: [N] out. */
+int ms_rambo_massless(int64_t N, int n, double sqrt_s, const double* d_sqrt_s, const double* d_x, ms_rng rng,
+                      double* d_p, double* d_w, int64_t ld, uint32_t* d_fail, void* stream);
+
+/* ms_fastrambo -- FastRambo (Eq. 64-67, Table 1): as above with Eq. 62 replaced by
+ * the rational-quadratic map, y_i = G_RQF^{-1}(x; c_k) (Eq. 65), u_i = y_i^{1/(2k)}, k = n-i; weight
+ * d_w[e] = Phi_n(sqrt_s) * prod_i (k+1)(1-y_i^{1/k})/g_RQF(y_i; c_k) (Eq. 67 / Eq. 63). */
+int ms_fastrambo(int64_t N, int n, double sqrt_s, const double* d_sqrt_s, const double* d_x, ms_rng rng,
+                 double* d_p, double* d_w, int64_t ld, uint32_t* d_fail, void* stream);
+
+/* ms_fastrambo_inverse -- analytic inverse of ms_fastrambo (Eq. 64; readings F-1..F-5).
+ * Reads the outgoing rows 8.. of d_p (any frame in which they were generated from Q_1 = sum p),
+ * writes d_x [3n-4][ld] and, if d_w != NULL, the same weight the forward map returns. */
+int ms_fastrambo_inverse(int64_t N, int n, const double* d_p, double* d_x, double* d_w, int64_t ld, void* stream);
+
+/* ms_massive_rescale -- massive extension, strategy (i) of PAPER.md:510 (momentum rescaling of classic
+ * RAMBO, ref. [64]; readings K-1..K-3): solve sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt_s for xi by Newton
+ * in registers until |F| <= rel_tol*sqrt_s (at most max_iter steps), k_i = (sqrt(m_i^2+xi^2 E_i^2), xi p_i),
+ * w_m = xi^(2n-3) sqrt_s prod(|k_i|/k_i^0) / sum(|k_i|^2/k_i^0).
+ * d_p: outgoing rows 8.. are read (massless, CM frame) and overwritten; incoming rows untouched.
+ * d_w: [N] multiplied in place by w_m.  h_masses: n doubles on the HOST. */
+int ms_massive_rescale(int64_t N, int n, double sqrt_s, const double* h_masses, double rel_tol, int max_iter,
+                       double* d_p, double* d_w, int64_t ld, uint32_t* d_fail, void* stream);
+
+/* ms_pdf_x_boost -- Bjorken-x sampling and lab boost (Eq. 19 with m^2=0, Eq. 21-23;
+ * ops r_to_x1x2 and boost_beam; readings X-1, X-2).
+ *   phase 0 (sample): tau = tau_min^(1-r_0), x1 = tau^r_1, x2 = tau^(1-r_1);
+ *       d_x1x2 [2][ld], d_sqrt_shat[N] = sqrt(tau s_had), d_jac[N] = tau ln(1/tau_min) ln(1/tau).
+ *       d_r = rows r_0, r_1 [2][ld] or NULL -> Philox j = 0,1.  d_p unused.
+ *   phase 1 (boost): outgoing rows of d_p are boosted along z from the partonic CM frame by
+ *       rapidity (1/2) ln(x1/x2); incoming rows are set to x_{1,2} (sqrt(s_had)/2)(1,0,0,+-1).
+ *       Reads d_x1x2; d_r, d_sqrt_shat, d_jac unused. */
+int ms_pdf_x_boost(int64_t N, int n, double s_had, double tau_min, int phase, const double* d_r, ms_rng rng,
+                   double* d_x1x2, double* d_sqrt_shat, double* d_jac, double* d_p, int64_t ld, void* stream);
+
+/* ms_toy_integrand -- BASELINE.json's matrix-element stand-in (not from the paper; reading T):
+ * f = prod_{i=1}^{n-1} 1/(s_{i,i+1} + reg), s_ij := E_i E_j |p_i/E_i - p_j/E_j|^2 over outgoing neighbours.
+ * d_f[e] = f, or d_f[e] *= f when accumulate != 0. */
+int ms_toy_integrand(int64_t N, int n, double reg, const double* d_p, double* d_f, int accumulate, int64_t ld,
+                     void* stream);
+
+/* ms_reduce_max -- *d_out = max(d_w[0..N-1]) (w_max of the pre-run, reading U).  d_out must be
+ * zero-initialised or hold a lower bound; weights are non-negative. */
+int ms_reduce_max(int64_t N, const double* d_w, double* d_out, void* stream);
+
+/* ms_unweight -- single-pass hit-or-miss unweighting against a fixed w_max (reading U)
+ * with stable stream compaction (warp ballot + block scan + decoupled look-back across tiles).
+ *   accept_e <=> u_e * w_max < w_e, u_e = Philox uniform j=0 of (rng.seed, rng.stream, event);
+ *   accepted events are written in increasing event order: d_idx[k] = e, d_w_out[k] = max(1, w_e/w_max),
+ *   d_rows_out[r*cap + k] = d_rows_in[r*ld + e] for r < n_rows (skipped if either pointer is NULL).
+ *   *d_n_accepted = true number accepted; only the first `cap` are stored.
+ * d_wmax: device scalar.  d_scratch: ms_unweight_scratch_bytes(N) bytes, any content (the call
+ * clears it on the stream). */
+size_t ms_unweight_scratch_bytes(int64_t N);
+int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, int n_rows, const double* d_rows_in,
+                int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted,
+                void* d_scratch, size_t scratch_bytes, int64_t ld, void* stream);
+
+/* ms_generate -- the fused hot path: Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [massive rescale]
+ * -> [lab boost] -> [toy integrand] -> weight, one thread per event, everything in registers, only the
+ * momenta and the weight are written.  Computes exactly what the chain
+ * ms_vegas_map, ms_pdf_x_boost(0), ms_rambo_massless|ms_fastrambo, ms_massive_rescale, ms_pdf_x_boost(1),
+ * ms_toy_integrand computes; d_w[e] = jac_VEGAS * w_PS [* J_x] [* w_m] [* f]. */
+typedef struct ms_gen_config {
+    int32_t n;             /* outgoing particles */
+    int32_t mapping;       /* 0 FastRambo, 1 exact Rambo */
+    int32_t grid_dims;     /* 0: no grid (uniforms used directly); else >= uniforms consumed */
+    int32_t grid_bins;
+    int32_t pdf;           /* 1: dims 0,1 -> (tau, y); phase space at sqrt(tau s_had); boost to lab */
+    int32_t massive;       /* 1: Newton rescale to `masses` */
+    int32_t toy;           /* 1: multiply the weight by the toy integrand */
+    int32_t max_iter;      /* Newton cap of the rescale */
+    double sqrt_s;         /* partonic (pdf=0) or hadronic (pdf=1) CM energy */
+    double tau_min;
+    double rel_tol;        /* rescale tolerance */
+    double toy_reg;
+    double masses[MS_MAX_N];
+} ms_gen_config;
+
+/* d_edges: [grid_dims][grid_bins+1] or NULL when grid_dims = 0.  d_p: [4(n+2)][ld].  d_w: [N].
+ * d_x1x2: [2][ld] or NULL (pdf only). */
+int ms_generate(const ms_gen_config* cfg, int64_t N, ms_rng rng, const double* d_edges, double* d_p, double* d_w,
+                double* d_x1x2, int64_t ld, uint32_t* d_fail, void* stream);
+
+/* ms_fill_uniforms -- materialise Philox uniforms j = 0..d-1 as rows d_r[d][ld] (step S0 on its own). */
+int ms_fill_uniforms(int64_t N, int d, ms_rng rng, double* d_r, int64_t ld, void* stream);
+
+/* ms_probe_dfma -- measurement helper: `iters` dependent-free DFMA chains per thread on `blocks` x 256
+ * threads; d_sink receives one double per thread.  Executes blocks*256*iters*8 DFMA. */
+int ms_probe_dfma(int blocks, int iters, double* d_sink, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MADSPACE_B200_H */

@@ -1,0 +1,201 @@
+"""paper_2602_06895_b200 -- B200-native (sm_100a) hot path of MadSpace (arXiv 2602.06895).
+
+Thin ctypes binding of ``libmadspace_b200.so`` (C ABI: ``include/madspace_b200.h``).  The functions here carry
+the SAME names as the C entry points and do argument marshalling only: every step of the path runs in the
+library's CUDA kernels.  PyTorch is used for device memory and streams, nothing else.  There is NO CPU
+fallback: if the library cannot be built/loaded the import of a function raises, and every call raises
+``MadSpaceError`` on a non-zero return code.
+
+Layout: structure of arrays, fp64, ``a[row, event]`` (C-contiguous torch tensors on the device); momentum
+row = 4*particle + mu with mu = (E, px, py, pz), particles 0,1 incoming, 2..n+1 outgoing.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass, field
+from typing import Optional, Sequence
+
+from . import _build
+
+MS_MAX_N = 9
+MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA = 0, -1, -2, -3, -4
+_ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA"}
+
+EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_rambo_massless", "ms_fastrambo",
+           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma")
+
+
+class MadSpaceError(RuntimeError):
+    def __init__(self, fn: str, code: int, cuda: int = 0):
+        self.code, self.cuda = code, cuda
+        super().__init__("%s failed: %s%s" % (fn, _ERR.get(code, str(code)),
+                                              " (cudaError %d)" % cuda if code == MS_ECUDA else ""))
+
+
+class ms_rng(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("stream", C.c_uint32), ("reserved", C.c_uint32), ("event_offset", C.c_uint64)]
+
+
+class ms_gen_config(C.Structure):
+    _fields_ = [("n", C.c_int32), ("mapping", C.c_int32), ("grid_dims", C.c_int32), ("grid_bins", C.c_int32),
+                ("pdf", C.c_int32), ("massive", C.c_int32), ("toy", C.c_int32), ("max_iter", C.c_int32),
+                ("sqrt_s", C.c_double), ("tau_min", C.c_double), ("rel_tol", C.c_double), ("toy_reg", C.c_double),
+                ("masses", C.c_double * MS_MAX_N)]
+
+
+_lib = None
+_vp, _i64, _int, _dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib() -> C.CDLL:
+    """Load (building first if the sources are newer) the CUDA library.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        L.ms_version.restype = C.c_char_p
+        L.ms_unweight_scratch_bytes.restype = C.c_size_t
+        L.ms_unweight_scratch_bytes.argtypes = [_i64]
+        L.ms_check_grid.argtypes = [_int, _int, _vp]
+        L.ms_fill_uniforms.argtypes = [_i64, _int, ms_rng, _vp, _i64, _vp]
+        L.ms_vegas_map.argtypes = [_i64, _int, _int, _vp, _int, _vp, ms_rng, _vp, _vp, _i64, _vp]
+        for name in ("ms_rambo_massless", "ms_fastrambo"):
+            getattr(L, name).argtypes = [_i64, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
+        L.ms_fastrambo_inverse.argtypes = [_i64, _int, _vp, _vp, _vp, _i64, _vp]
+        L.ms_massive_rescale.argtypes = [_i64, _int, _dbl, _vp, _dbl, _int, _vp, _vp, _i64, _vp, _vp]
+        L.ms_pdf_x_boost.argtypes = [_i64, _int, _dbl, _dbl, _int, _vp, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp]
+        L.ms_toy_integrand.argtypes = [_i64, _int, _dbl, _vp, _vp, _int, _i64, _vp]
+        L.ms_reduce_max.argtypes = [_i64, _vp, _vp, _vp]
+        L.ms_unweight.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
+        L.ms_generate.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp]
+        L.ms_probe_dfma.argtypes = [_int, _int, _vp, _vp]
+        _lib = L
+    return _lib
+
+
+def _ptr(t) -> Optional[int]:
+    """Device (or host) address of a torch tensor / numpy array / raw int; None stays NULL."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _check(fn: str, rc: int) -> None:
+    if rc != MS_OK:
+        raise MadSpaceError(fn, rc, lib().ms_last_cuda_error() if rc == MS_ECUDA else 0)
+
+
+def rng(seed: int, stream: int = 0, event_offset: int = 0) -> ms_rng:
+    return ms_rng(seed, stream, 0, event_offset)
+
+
+# ----------------------------------------------------------------------------------------------- C ABI mirrors
+
+def ms_version() -> str:
+    return lib().ms_version().decode()
+
+
+def ms_last_cuda_error() -> int:
+    return int(lib().ms_last_cuda_error())
+
+
+def ms_check_grid(h_edges) -> int:
+    """h_edges: numpy float64 [d][n_bins+1] on the host.  Returns the code (does not raise on MS_EGRID)."""
+    d, nb1 = h_edges.shape
+    return int(lib().ms_check_grid(d, nb1 - 1, h_edges.ctypes.data))
+
+
+def ms_fill_uniforms(N, d, r: ms_rng, d_r, ld, stream=None) -> None:
+    _check("ms_fill_uniforms", lib().ms_fill_uniforms(N, d, r, _ptr(d_r), ld, _stream(stream)))
+
+
+def ms_vegas_map(N, d, n_bins, d_edges, direction, d_in, r: ms_rng, d_out, d_jac, ld, stream=None) -> None:
+    _check("ms_vegas_map", lib().ms_vegas_map(N, d, n_bins, _ptr(d_edges), direction, _ptr(d_in), r, _ptr(d_out),
+                                              _ptr(d_jac), ld, _stream(stream)))
+
+
+def ms_rambo_massless(N, n, sqrt_s, d_sqrt_s, d_x, r: ms_rng, d_p, d_w, ld, d_fail=None, stream=None) -> None:
+    _check("ms_rambo_massless", lib().ms_rambo_massless(N, n, sqrt_s, _ptr(d_sqrt_s), _ptr(d_x), r, _ptr(d_p), _ptr(d_w),
+                                                        ld, _ptr(d_fail), _stream(stream)))
+
+
+def ms_fastrambo(N, n, sqrt_s, d_sqrt_s, d_x, r: ms_rng, d_p, d_w, ld, d_fail=None, stream=None) -> None:
+    _check("ms_fastrambo", lib().ms_fastrambo(N, n, sqrt_s, _ptr(d_sqrt_s), _ptr(d_x), r, _ptr(d_p), _ptr(d_w), ld,
+                                              _ptr(d_fail), _stream(stream)))
+
+
+def ms_fastrambo_inverse(N, n, d_p, d_x, d_w, ld, stream=None) -> None:
+    _check("ms_fastrambo_inverse", lib().ms_fastrambo_inverse(N, n, _ptr(d_p), _ptr(d_x), _ptr(d_w), ld, _stream(stream)))
+
+
+def ms_massive_rescale(N, n, sqrt_s, masses: Sequence[float], rel_tol, max_iter, d_p, d_w, ld, d_fail=None,
+                       stream=None) -> None:
+    h = (C.c_double * len(masses))(*[float(m) for m in masses])
+    if len(masses) != n:
+        raise MadSpaceError("ms_massive_rescale", MS_EINVAL)
+    _check("ms_massive_rescale", lib().ms_massive_rescale(N, n, sqrt_s, C.addressof(h), rel_tol, max_iter, _ptr(d_p),
+                                                          _ptr(d_w), ld, _ptr(d_fail), _stream(stream)))
+
+
+def ms_pdf_x_boost(N, n, s_had, tau_min, phase, d_r, r: ms_rng, d_x1x2, d_sqrt_shat, d_jac, d_p, ld, stream=None) -> None:
+    _check("ms_pdf_x_boost", lib().ms_pdf_x_boost(N, n, s_had, tau_min, phase, _ptr(d_r), r, _ptr(d_x1x2),
+                                                  _ptr(d_sqrt_shat), _ptr(d_jac), _ptr(d_p), ld, _stream(stream)))
+
+
+def ms_toy_integrand(N, n, reg, d_p, d_f, accumulate, ld, stream=None) -> None:
+    _check("ms_toy_integrand", lib().ms_toy_integrand(N, n, reg, _ptr(d_p), _ptr(d_f), int(accumulate), ld, _stream(stream)))
+
+
+def ms_reduce_max(N, d_w, d_out, stream=None) -> None:
+    _check("ms_reduce_max", lib().ms_reduce_max(N, _ptr(d_w), _ptr(d_out), _stream(stream)))
+
+
+def ms_unweight_scratch_bytes(N) -> int:
+    return int(lib().ms_unweight_scratch_bytes(N))
+
+
+def ms_unweight(N, d_w, d_wmax, r: ms_rng, n_rows, d_rows_in, cap, d_idx, d_w_out, d_rows_out, d_n_accepted, d_scratch,
+                scratch_bytes, ld, stream=None) -> None:
+    _check("ms_unweight", lib().ms_unweight(N, _ptr(d_w), _ptr(d_wmax), r, n_rows, _ptr(d_rows_in), cap, _ptr(d_idx),
+                                            _ptr(d_w_out), _ptr(d_rows_out), _ptr(d_n_accepted), _ptr(d_scratch),
+                                            scratch_bytes, ld, _stream(stream)))
+
+
+def gen_config(n, mapping="fastrambo", sqrt_s=0.0, grid_dims=0, grid_bins=0, pdf=False, tau_min=0.0, masses=(),
+               rel_tol=1e-14, max_iter=10, toy=False, toy_reg=100.0) -> ms_gen_config:
+    cfg = ms_gen_config()
+    cfg.n, cfg.mapping = n, {"fastrambo": 0, "rambo": 1}[mapping]
+    cfg.grid_dims, cfg.grid_bins = grid_dims, grid_bins
+    cfg.pdf, cfg.massive, cfg.toy, cfg.max_iter = int(pdf), int(len(masses) > 0), int(toy), max_iter
+    cfg.sqrt_s, cfg.tau_min, cfg.rel_tol, cfg.toy_reg = sqrt_s, tau_min, rel_tol, toy_reg
+    for i, m in enumerate(masses):
+        cfg.masses[i] = float(m)
+    return cfg
+
+
+def ms_generate(cfg: ms_gen_config, N, r: ms_rng, d_edges, d_p, d_w, d_x1x2, ld, d_fail=None, stream=None) -> None:
+    _check("ms_generate", lib().ms_generate(C.byref(cfg), N, r, _ptr(d_edges), _ptr(d_p), _ptr(d_w), _ptr(d_x1x2), ld,
+                                            _ptr(d_fail), _stream(stream)))
+
+
+def ms_probe_dfma(blocks, iters, d_sink, stream=None) -> None:
+    _check("ms_probe_dfma", lib().ms_probe_dfma(blocks, iters, _ptr(d_sink), _stream(stream)))

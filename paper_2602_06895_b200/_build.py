@@ -1,0 +1,69 @@
+"""In-tree build of libmadspace_b200.so with nvcc for sm_100a (no torch types, no JIT cache).
+
+The per-multiplicity kernels (csrc/ms_inst.cu, -DMS_N=2..9) compile as eight translation units in parallel;
+csrc/ms_api.cu holds the C ABI.  Objects live in csrc/build/ (git-ignored); the shared library lands beside
+this file so that it travels to the GPU box with the repository snapshot.
+"""
+from __future__ import annotations
+
+import concurrent.futures as cf
+import os
+import shutil
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(_HERE, "csrc")
+BUILD = os.path.join(CSRC, "build")
+INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
+LIB = os.path.join(_HERE, "libmadspace_b200.so")
+
+NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-diag-suppress", "177"]
+HEADERS = ["ms_math.cuh", "ms_kernels.cuh", "ms_params.h", "ms_launch.h"]
+N_RANGE = range(2, 10)
+
+
+def _nvcc() -> str:
+    exe = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(exe):
+        raise RuntimeError("nvcc not found: the CUDA path cannot be built (there is no CPU fallback)")
+    return exe
+
+
+def _newest_source() -> float:
+    files = [os.path.join(CSRC, f) for f in HEADERS + ["ms_inst.cu", "ms_api.cu"]]
+    files.append(os.path.join(INCLUDE, "madspace_b200.h"))
+    return max(os.path.getmtime(f) for f in files)
+
+
+def _compile(args):
+    src, obj, extra = args
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + ["-c", src, "-o", obj]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    return obj
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
+        return LIB
+    os.makedirs(BUILD, exist_ok=True)
+    jobs = [(os.path.join(CSRC, "ms_api.cu"), os.path.join(BUILD, "ms_api.o"), ["-I", INCLUDE])]
+    for n in N_RANGE:
+        jobs.append((os.path.join(CSRC, "ms_inst.cu"), os.path.join(BUILD, "ms_inst_n%d.o" % n), ["-DMS_N=%d" % n]))
+    with cf.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+        objs = list(ex.map(_compile, jobs))
+    tmp = LIB + ".tmp.%d" % os.getpid()
+    cmd = [_nvcc(), "-shared", "-o", tmp] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("link failed: %s\n%s" % (r.stdout, r.stderr))
+    os.replace(tmp, LIB)
+    if verbose:
+        print("built", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    build(force=True, verbose=True)

@@ -1,0 +1,56 @@
+// ms_params.h -- plain-data launch parameters shared by the host API (ms_api.cu) and the kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ms {
+
+constexpr int kBlock = 256;
+constexpr int kMaxN = 9;
+
+struct PhiloxKey {
+    uint32_t k0, k1, stream;
+    uint64_t event_offset;
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Launch parameters (plain data, passed by value as a __grid_constant__).
+// ---------------------------------------------------------------------------------------------------
+struct GenParams {
+    int64_t N, ld;
+    PhiloxKey key;
+    const double* x_rows;      // [d][ld] uniforms, or nullptr -> Philox in-kernel
+    const double* sqrt_s_arr;  // per-event CM energy, or nullptr
+    const double* edges;       // VEGAS edges [grid_dims][grid_bins+1], or nullptr
+    int grid_dims, grid_bins;
+    int pdf, toy, max_iter, _pad;
+    double sqrt_s;             // fixed CM energy (partonic), or hadronic sqrt(s_had) when pdf
+    double phi_unit;           // Phi_n(1), Eq. 81
+    double phi_fixed;          // Phi_n(sqrt_s) when the energy is fixed
+    double ln_tau_min, rel_tol, toy_reg;
+    double masses[kMaxN];
+    double* p;                 // [4(n+2)][ld]
+    double* w;                 // [N]
+    double* x1x2;              // [2][ld] or nullptr
+    uint32_t* fail;
+};
+
+struct InvParams {
+    int64_t N, ld;
+    const double* p;
+    double* x;
+    double* w;                 // or nullptr
+    double phi_unit;
+};
+
+struct RescaleParams {
+    int64_t N, ld;
+    double sqrt_s, rel_tol;
+    int max_iter, _pad;
+    double masses[kMaxN];
+    double* p;
+    double* w;
+    uint32_t* fail;
+};
+
+}  // namespace ms

@@ -1,0 +1,128 @@
+"""HotPath -- device buffers plus the call sequence of one pass of the hot path (what bench.py times and the
+tests check).  Marshalling and buffer ownership only: every arithmetic step is a call into the C ABI.
+
+One step = ms_generate (Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [rescale] -> [boost] -> [toy] -> weight)
+           [-> ms_reduce_max over the pre-run events -> ms_unweight (accept + stable compaction)]
+           [-> ms_fastrambo_inverse -> ms_vegas_map(inverse)]            (round trip, cfg 5)
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import (gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
+               ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID)
+
+
+@dataclass
+class PathSpec:
+    """What one step computes (mirrors ms_gen_config plus the unweighting / round-trip stages)."""
+    n: int
+    sqrt_s: float
+    mapping: str = "fastrambo"            # "fastrambo" | "rambo"
+    edges: Optional[np.ndarray] = None    # host VEGAS table [d][n_bins+1] or None
+    pdf: bool = False
+    tau_min: float = 0.0
+    masses: Sequence[float] = ()
+    toy: bool = False
+    toy_reg: float = 100.0
+    unweight: bool = False
+    inverse: bool = False
+    prerun: int = 1 << 16                 # w_max = max weight of events 0..prerun-1 (reading U)
+    seed_events: int = 1
+    seed_unweight: int = 3
+    rel_tol: float = 1e-14
+    max_iter: int = 10
+
+    @property
+    def d_used(self) -> int:
+        return 3 * self.n - 4 + (2 if self.pdf else 0)
+
+    @property
+    def rows_p(self) -> int:
+        return 4 * (self.n + 2)
+
+
+class HotPath:
+    def __init__(self, spec: PathSpec, N: int, device="cuda:0", cap: Optional[int] = None, gather_rows: bool = True):
+        if not torch.cuda.is_available():
+            raise RuntimeError("HotPath needs a CUDA device: there is no CPU fallback")
+        self.spec, self.N, self.device = spec, int(N), torch.device(device)
+        self.ld = (self.N + 1) // 2 * 2                      # even row stride keeps every row 16-byte aligned
+        f64 = dict(dtype=torch.float64, device=self.device)
+        self.p = torch.empty((spec.rows_p, self.ld), **f64)
+        self.w = torch.empty(self.ld, **f64)
+        self.x1x2 = torch.empty((2, self.ld), **f64) if spec.pdf else None
+        self.fail = torch.zeros(1, dtype=torch.int32, device=self.device)
+        self.d_edges = None
+        self.grid_dims = self.grid_bins = 0
+        if spec.edges is not None:
+            self.set_grid(spec.edges)
+        self.cfg = gen_config(spec.n, spec.mapping, spec.sqrt_s, self.grid_dims, self.grid_bins, spec.pdf, spec.tau_min,
+                              tuple(spec.masses), spec.rel_tol, spec.max_iter, spec.toy, spec.toy_reg)
+        if spec.unweight:
+            self.cap = int(cap) if cap is not None else max(1024, self.N // 64)
+            self.wmax = torch.zeros(1, **f64)
+            self.idx = torch.empty(self.cap, dtype=torch.int64, device=self.device)
+            self.w_out = torch.empty(self.cap, **f64)
+            self.gather_rows = gather_rows
+            self.rows_out = torch.empty((spec.rows_p, self.cap), **f64) if gather_rows else None
+            self.n_acc = torch.zeros(1, dtype=torch.int64, device=self.device)
+            self.scratch_bytes = ms_unweight_scratch_bytes(self.N)
+            self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
+        if spec.inverse:
+            self.d_inv = 3 * spec.n - 4
+            self.x_inv = torch.empty((self.d_inv, self.ld), **f64)
+            self.w_inv = torch.empty(self.ld, **f64)
+            self.r_inv = torch.empty((self.d_inv, self.ld), **f64) if self.d_edges is not None else None
+
+    def set_grid(self, h_edges: np.ndarray) -> None:
+        h_edges = np.ascontiguousarray(h_edges, dtype=np.float64)
+        if ms_check_grid(h_edges) != 0:
+            raise MadSpaceError("ms_check_grid", MS_EGRID)
+        self.grid_dims, self.grid_bins = h_edges.shape[0], h_edges.shape[1] - 1
+        t = torch.from_numpy(h_edges)
+        if self.d_edges is None:
+            self.d_edges = torch.empty(h_edges.shape, dtype=torch.float64, device=self.device)
+        self.d_edges.copy_(t, non_blocking=True)
+
+    # ---- stages -------------------------------------------------------------------------------
+    def generate(self, event_offset: int = 0, stream=None) -> None:
+        ms_generate(self.cfg, self.N, rng(self.spec.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
+                    self.x1x2, self.ld, self.fail, stream)
+
+    def unweight(self, event_offset: int = 0, stream=None) -> None:
+        s = self.spec
+        self.wmax.zero_()
+        ms_reduce_max(min(s.prerun, self.N), self.w, self.wmax, stream)
+        ms_unweight(self.N, self.w, self.wmax, rng(s.seed_unweight, 1, event_offset), s.rows_p if self.gather_rows else 0,
+                    self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
+                    self.scratch, self.scratch_bytes, self.ld, stream)
+
+    def invert(self, stream=None) -> None:
+        s = self.spec
+        ms_fastrambo_inverse(self.N, s.n, self.p, self.x_inv, self.w_inv, self.ld, stream)
+        if self.d_edges is not None:
+            # only the dimensions the phase-space map consumed are inverted
+            ms_vegas_map(self.N, self.d_inv, self.grid_bins, self.d_edges, 1, self.x_inv, rng(0), self.r_inv, None,
+                         self.ld, stream)
+
+    def step(self, event_offset: int = 0, stream=None) -> None:
+        self.generate(event_offset, stream)
+        if self.spec.unweight:
+            self.unweight(event_offset, stream)
+        if self.spec.inverse:
+            self.invert(stream)
+
+    @property
+    def launches_per_step(self) -> int:
+        """Kernels of this library enqueued by one step() (memsets/copies not counted)."""
+        k = 1
+        if self.spec.unweight:
+            k += 2
+        if self.spec.inverse:
+            k += 2 if self.d_edges is not None else 1
+        return k
