@@ -1,0 +1,369 @@
+#!/usr/bin/env python
+"""bench.py -- phase-space events/s of the MadSpace hot path on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
+
+A step = one pass of the whole hot path over one batch of synthetic (Philox-seeded) events: for the default
+workload (BASELINE.json configs[1], "cfg2": massless 2->4 FastRambo, 2^24 events, seeded 128x8 VEGAS grid, toy
+integrand, unweighting) that is ms_generate -> ms_reduce_max (pre-run w_max) -> ms_unweight.
+N > 1 (torchrun): one process per GPU, every rank generates its own 2^24-event batch at event offset rank*2^24
+(weak scaling, no data-path collective); value = events of all ranks / max-over-ranks time.
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import ms_inputs  # noqa: E402
+
+METRIC = "phase-space events/s (fp64, weighted events through the whole hot path)"
+UNIT = "events/s"
+FP64_LANES_PER_SM = 64            # B200 (GB100): 64 FP64 FMA lanes per SM (datasheet 37 TFLOP/s = 148*64*2*1.965 GHz)
+
+# Hand-counted fp64-pipe instructions of the final formulas: per stage.
+ALG_FP64 = {"vegas_dim": 6, "fast_mass": 96, "exact_mass_k1": 40, "exact_mass": 150, "decay": 64, "decay_first": 44,
+            "toy_pair": 15, "toy_particle": 11, "weight": 14, "pdf": 75, "boost_particle": 4,
+            "rescale_iter_massive": 16, "rescale_iter_massless": 2, "rescale_fixed": 40}
+
+
+def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
+    n = wl.n
+    c = ALG_FP64["vegas_dim"] * wl.grid_dims
+    if wl.mapping == "fastrambo":
+        c += ALG_FP64["fast_mass"] * (n - 2)
+    else:
+        c += ALG_FP64["exact_mass"] * max(n - 3, 0) + (ALG_FP64["exact_mass_k1"] if n > 2 else 0)
+    c += ALG_FP64["decay_first"] + ALG_FP64["decay"] * (n - 2)
+    if wl.toy:
+        c += ALG_FP64["toy_particle"] * n + ALG_FP64["toy_pair"] * (n - 1)
+    if wl.pdf:
+        c += ALG_FP64["pdf"] + ALG_FP64["boost_particle"] * n
+    if wl.masses:
+        nm = sum(1 for m in wl.masses if m > 0)
+        c += ALG_FP64["rescale_fixed"] + 4 * (ALG_FP64["rescale_iter_massive"] * nm + ALG_FP64["rescale_iter_massless"] * (n - nm) + 12)
+    return c + ALG_FP64["weight"]
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi sampled DURING the timed region (profiling recipe's clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle arm
+
+def oracle_step(orc, wl, n_events, offset=0):
+    """One pass of the same hot path over `n_events` events with the oracle as it stands (tests/helpers.py chain +
+    w_max of the pre-run + sequential hit-or-miss unweighting [+ inverse round trip])."""
+    from oracle.chain import oracle_chain
+    ref = oracle_chain(orc, wl, np.arange(offset, offset + n_events))
+    n_acc = None
+    if wl.unweight:
+        w = np.ascontiguousarray(ref["w"])
+        wmax = orc.wmax(np.ascontiguousarray(w[:min(ms_inputs.PRERUN, n_events)]))
+        _, _, n_acc = orc.unweight(w, wmax, ms_inputs.SEED_UNWEIGHT, ms_inputs.STREAM_UNWEIGHT, offset, n_events)
+    if wl.inverse:
+        xi, _ = orc.fastrambo_inverse(wl.n, ref["p"])
+        edges = wl.grid()
+        if edges is not None:
+            orc.vegas_inverse(np.ascontiguousarray(edges[:3 * wl.n - 4]), xi)
+    return n_acc
+
+
+def time_oracle(wl, target_seconds=12.0, steps=1, warmup=0):
+    import oracle as orc
+    orc.lib()
+    probe = 1 << 16
+    t0 = time.perf_counter()
+    oracle_step(orc, wl, probe)
+    t_probe = max(time.perf_counter() - t0, 1e-4)
+    per_step = target_seconds / max(steps + warmup, 1)
+    n = int(min(wl.N, max(probe, probe * per_step / t_probe)))
+    n = 1 << (n.bit_length() - 1)
+    for _ in range(warmup):
+        oracle_step(orc, wl, n)
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        oracle_step(orc, wl, n)
+        times.append(time.perf_counter() - t0)
+    t = float(np.mean(times))
+    return {"value": n / t, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "first %d events (2^%d) of %s per step, %d step(s); OpenMP over event ranges, sequential unweighting"
+                      % (n, n.bit_length() - 1, wl.name, steps)}, t
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = ms_inputs.WORKLOADS[args.workload]
+    cb, t = time_oracle(wl, target_seconds=60.0, steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(wl, args.gpus), "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(wl, n_gpus):
+    return {"workload": "%s: %s" % (wl.name, wl.note), "events_per_gpu_per_step": wl.N, "n": wl.n,
+            "grid": "%dx%d %s" % (wl.grid_bins, wl.grid_dims, wl.grid_kind), "parallelism": "events sharded x%d" % n_gpus,
+            "l2": "no flush needed: each step streams %.2f GB of fresh output (> 126 MB L2)" % (wl.N * wl.out_bytes_per_event / 1e9)}
+
+
+# ------------------------------------------------------------------------------------------------ GPU arm
+
+def spec_from_workload(wl):
+    from paper_2602_06895_b200.pipeline import PathSpec
+    return PathSpec(n=wl.n, sqrt_s=wl.sqrt_s, mapping=wl.mapping, edges=wl.grid(), pdf=wl.pdf, tau_min=wl.tau_min,
+                    masses=tuple(wl.masses), toy=wl.toy, toy_reg=ms_inputs.TOY_REG, unweight=wl.unweight,
+                    inverse=wl.inverse, prerun=ms_inputs.PRERUN, seed_events=ms_inputs.SEED_EVENTS,
+                    seed_unweight=ms_inputs.SEED_UNWEIGHT)
+
+
+def probe_fp64_rate(ms, torch, seconds=0.25):
+    """Sustained DFMA issue rate (instructions/s) measured with ms_probe_dfma: 8 independent chains per thread."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    blocks, iters = sms * 8, 1 << 14
+    sink = torch.empty(blocks * 256, dtype=torch.float64, device="cuda")
+    ms.ms_probe_dfma(blocks, iters, sink)
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps, best, t_end = 0, 0.0, time.perf_counter() + seconds
+    while time.perf_counter() < t_end or reps < 3:
+        ev0.record()
+        ms.ms_probe_dfma(blocks, iters, sink)
+        ev1.record()
+        ev1.synchronize()
+        best = max(best, blocks * 256 * iters * 8 / (ev0.elapsed_time(ev1) * 1e-3))
+        reps += 1
+    return best
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2602_06895_b200 as ms
+    from paper_2602_06895_b200.pipeline import HotPath
+    from paper_2602_06895_b200.sharding import gather_counts, output_offsets, weak_range
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference for the oracle)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ms.lib()
+    wl = ms_inputs.WORKLOADS[args.workload]
+    N = wl.N if args.events <= 0 else args.events
+    offset, _ = weak_range(N, rank)
+    dev = torch.device("cuda", local)
+    hp = HotPath(spec_from_workload(wl), N, dev, cap=max(1 << 16, N // 256))
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between barriers + synchronize
+    for _ in range(args.warmup):
+        hp.step(offset)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    gen_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev[0].record(stream)
+    for k in range(args.steps):
+        gen_ev[k][0].record(stream)
+        hp.generate(offset)
+        gen_ev[k][1].record(stream)
+        if wl.unweight:
+            hp.unweight(offset)
+        if wl.inverse:
+            hp.invert()
+    ev[1].record(stream)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    t_total = ev[0].elapsed_time(ev[1]) * 1e-3
+    t_gen = float(np.mean([a.elapsed_time(b) for a, b in gen_ev])) * 1e-3
+    n_acc_local = int(hp.n_acc.item()) if wl.unweight else 0
+    if world > 1:
+        tt = torch.tensor([t_total, t_gen], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_total, t_gen = float(tt[0]), float(tt[1])
+    counts = gather_counts(n_acc_local)
+    offsets = output_offsets(counts)
+
+    # ---- end to end through the C ABI with HOST buffers: grid table H2D and the unweighted sample D2H every step
+    h_edges = torch.from_numpy(wl.grid()).pin_memory() if wl.grid() is not None else None
+    d2h = []
+    if wl.unweight:
+        d2h = [(hp.n_acc, torch.empty(1, dtype=torch.int64).pin_memory()),
+               (hp.idx, torch.empty(hp.cap, dtype=torch.int64).pin_memory()),
+               (hp.w_out, torch.empty(hp.cap, dtype=torch.float64).pin_memory()),
+               (hp.rows_out, torch.empty((hp.spec.rows_p, hp.cap), dtype=torch.float64).pin_memory())]
+    else:
+        d2h = [(hp.w, torch.empty(hp.ld, dtype=torch.float64).pin_memory()),
+               (hp.p, torch.empty((hp.spec.rows_p, hp.ld), dtype=torch.float64).pin_memory())]
+    h2d_bytes = h_edges.numel() * 8 if h_edges is not None else 0
+    d2h_bytes = sum(h.numel() * h.element_size() for _, h in d2h)
+
+    def e2e_step():
+        if h_edges is not None:
+            hp.d_edges.copy_(h_edges, non_blocking=True)
+        hp.step(offset)
+        for d, h in d2h:
+            h.copy_(d, non_blocking=True)
+        torch.cuda.current_stream().synchronize()          # the host consumes the step's result
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    ev[0].record(stream)
+    for _ in range(args.steps):
+        e2e_step()
+    ev[1].record(stream)
+    barrier()
+    t_e2e = max(ev[0].elapsed_time(ev[1]) * 1e-3, 0.0)
+    t_e2e_wall = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = float(tt[0])
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (the fused generation kernel)
+    hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    bytes_per_launch = N * wl.out_bytes_per_event + (h2d_bytes if h_edges is not None else 0)
+    inst_per_event = alg_fp64_per_event(wl)
+    fp64_peak = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6            # fp64-pipe instructions / s at max clock
+    fp64_probe = probe_fp64_rate(ms, torch)
+    t_hbm = bytes_per_launch / (hbm_gbs * 1e9)
+    t_alu = N * inst_per_event / fp64_peak
+    if t_hbm >= t_alu:
+        roof = {"bound": "hbm", "achieved": bytes_per_launch / t_gen / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+    else:
+        roof = {"bound": "alu", "achieved": N * inst_per_event / t_gen / 1e9, "peak": fp64_peak / 1e9, "unit": "Ginst/s (fp64 pipe)"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof.update(traffic=args.traffic if args.traffic > 0 else None, kernel="ms::gen_kernel<%d,%s,%s>" % (
+        wl.n, "exact" if wl.mapping == "rambo" else "fast", "massive" if wl.masses else "massless"),
+        kernel_ms=1e3 * t_gen, kernel_share_of_step=t_gen * args.steps / t_total, peak_source=peak_src,
+        alg_bytes_per_event=wl.out_bytes_per_event, alg_fp64_inst_per_event=inst_per_event,
+        hbm_time_ms=1e3 * t_hbm, alu_time_ms=1e3 * t_alu, frac_of_max_side=max(t_hbm, t_alu) / t_gen,
+        fp64_peak_ginst_nominal=fp64_peak / 1e9, fp64_ginst_probe_measured=fp64_probe / 1e9,
+        kernel_events_per_s=N / t_gen)
+
+    cb = None if args.skip_cpu_baseline else time_oracle(wl, target_seconds=12.0)[0]
+    total_events = float(N) * world * args.steps
+    line = {"metric": METRIC, "value": total_events / t_total, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic (Philox-seeded uniforms; seeded VEGAS grid stands in for an adapted one)",
+            "config": workload_config(wl, world), "clocks": clocks,
+            "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+                    "wall_value": total_events / t_e2e_wall,
+                    "what": "grid table H2D from pinned memory + whole step + D2H of %s, host waits every step"
+                            % ("the accepted count and the compacted unweighted sample (idx, w_out, momentum rows; cap %d)" % hp.cap
+                               if wl.unweight else "all momenta and weights")},
+            "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "cpu_baseline": cb,
+            "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
+                            "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
+            "fail_count": int(hp.fail.item()),
+            "paper_context": "PAPER.md:766-770: full LO chain incl. matrix elements ~30M weighted evt/s on A100 (DY+1g), up to 10M on 24 Xeon-4214 cores; not this path in isolation"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg2", choices=sorted(ms_inputs.WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--events", type=int, default=0, help="override events per GPU per step (0 = the workload's)")
+    ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: do not time the oracle")
+    ap.add_argument("--traffic", type=float, default=0.0, help="dram bytes per launch of the dominant kernel from ncu (recorded, not measured here)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
