@@ -1,6 +1,6 @@
 """In-tree build of libmadspace_b200.so with nvcc for sm_100a (no torch types, no JIT cache).
 
-The per-multiplicity kernels (csrc/ms_inst.cu, -DMS_N=2..9) compile as eight translation units in parallel;
+The per-multiplicity kernels (csrc/ms_inst.cu, -DMS_N=2..9 -DMS_PART=0..2) compile as 24 translation units in parallel;
 csrc/ms_api.cu holds the C ABI.  Objects live in csrc/build/ (git-ignored); the shared library lands beside
 this file so that it travels to the GPU box with the repository snapshot.
 """
@@ -20,7 +20,7 @@ LIB = os.path.join(_HERE, "libmadspace_b200.so")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-diag-suppress", "177"]
 HEADERS = ["ms_math.cuh", "ms_kernels.cuh", "ms_params.h", "ms_launch.h"]
-N_RANGE = range(2, 10)
+N_RANGE = range(9, 1, -1)
 
 
 def _nvcc() -> str:
@@ -50,9 +50,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(BUILD, exist_ok=True)
     jobs = [(os.path.join(CSRC, "ms_api.cu"), os.path.join(BUILD, "ms_api.o"), ["-I", INCLUDE])]
-    for n in N_RANGE:
-        jobs.append((os.path.join(CSRC, "ms_inst.cu"), os.path.join(BUILD, "ms_inst_n%d.o" % n), ["-DMS_N=%d" % n]))
-    with cf.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+    for n in N_RANGE:                                  # largest multiplicities first: they take longest
+        for part in (0, 1, 2):
+            jobs.append((os.path.join(CSRC, "ms_inst.cu"), os.path.join(BUILD, "ms_inst_n%d_p%d.o" % (n, part)),
+                         ["-DMS_N=%d" % n, "-DMS_PART=%d" % part]))
+    with cf.ThreadPoolExecutor(max_workers=min(len(jobs), max(os.cpu_count() or 4, 4))) as ex:
         objs = list(ex.map(_compile, jobs))
     tmp = LIB + ".tmp.%d" % os.getpid()
     cmd = [_nvcc(), "-shared", "-o", tmp] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"]

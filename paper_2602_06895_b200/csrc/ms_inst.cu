@@ -1,10 +1,12 @@
-// ms_inst.cu -- compiled once per multiplicity (-DMS_N=2..9): instantiates the per-n kernels and exports one
-// launcher each, so that the eight translation units build in parallel.
+// ms_inst.cu -- compiled per multiplicity and part (-DMS_N=2..9 -DMS_PART=0|1|2): instantiates the per-n kernels and
+// exports one launcher each, so that the translation units build in parallel.
+//   part 0: generation kernels with the FastRambo mass chain; part 1: with the exact Rambo mass chain;
+//   part 2: FastRambo inverse and stand-alone massive rescale.
 #include "ms_kernels.cuh"
 #include "ms_launch.h"
 
-#ifndef MS_N
-#error "compile with -DMS_N=<n>"
+#if !defined(MS_N) || !defined(MS_PART)
+#error "compile with -DMS_N=<n> -DMS_PART=<0|1|2>"
 #endif
 
 namespace ms {
@@ -22,11 +24,17 @@ static int grid_for(K kernel, int64_t N, size_t smem)
     return (int)(tiles < resident ? tiles : resident);
 }
 
-template <bool EXACT, bool MASSIVE>
+#define MS_CAT2(a, b) a##b
+#define MS_CAT(a, b) MS_CAT2(a, b)
+
+#if MS_PART == 0 || MS_PART == 1
+constexpr bool kExact = MS_PART == 1;
+
+template <bool MASSIVE, bool PDF, bool TOY, bool ROWS, bool GRID>
 static cudaError_t launch_gen_t(const GenParams& P, cudaStream_t stream)
 {
-    auto kernel = gen_kernel<MS_N, EXACT, MASSIVE>;
-    const size_t smem = P.grid_dims > 0 ? (size_t)P.grid_dims * P.grid_bins * sizeof(double2) : 0;
+    auto kernel = gen_kernel<MS_N, kExact, MASSIVE, PDF, TOY, ROWS, GRID>;
+    const size_t smem = GRID ? (size_t)P.grid_dims * P.grid_bins * sizeof(double2) : 0;
     if (smem > 48 * 1024) {
         cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
@@ -35,15 +43,25 @@ static cudaError_t launch_gen_t(const GenParams& P, cudaStream_t stream)
     return cudaGetLastError();
 }
 
-#define MS_CAT2(a, b) a##b
-#define MS_CAT(a, b) MS_CAT2(a, b)
-
-cudaError_t MS_CAT(launch_gen_, MS_N)(const GenParams& P, bool exact, bool massive, cudaStream_t stream)
+#if MS_PART == 0
+cudaError_t MS_CAT(launch_gen_fast_, MS_N)
+#else
+cudaError_t MS_CAT(launch_gen_exact_, MS_N)
+#endif
+    (const GenParams& P, bool massive, bool pdf, bool toy, cudaStream_t stream)
 {
-    if (exact) return massive ? launch_gen_t<true, true>(P, stream) : launch_gen_t<true, false>(P, stream);
-    return massive ? launch_gen_t<false, true>(P, stream) : launch_gen_t<false, false>(P, stream);
+    if (P.x_rows != nullptr) return launch_gen_t<false, false, false, true, false>(P, stream);
+    const int sel = (P.grid_dims > 0 ? 8 : 0) | (massive ? 4 : 0) | (pdf ? 2 : 0) | (toy ? 1 : 0);
+#define MS_CASE(v) \
+    case v: return launch_gen_t<((v) & 4) != 0, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 8) != 0>(P, stream);
+    switch (sel) {
+        MS_CASE(0) MS_CASE(1) MS_CASE(2) MS_CASE(3) MS_CASE(4) MS_CASE(5) MS_CASE(6) MS_CASE(7)
+        MS_CASE(8) MS_CASE(9) MS_CASE(10) MS_CASE(11) MS_CASE(12) MS_CASE(13) MS_CASE(14) MS_CASE(15)
+        default: return cudaErrorInvalidValue;
+    }
+#undef MS_CASE
 }
-
+#else
 cudaError_t MS_CAT(launch_inverse_, MS_N)(const InvParams& P, cudaStream_t stream)
 {
     auto kernel = inverse_kernel<MS_N>;
@@ -57,5 +75,6 @@ cudaError_t MS_CAT(launch_rescale_, MS_N)(const RescaleParams& P, cudaStream_t s
     kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
     return cudaGetLastError();
 }
+#endif
 
 }  // namespace ms

@@ -32,12 +32,13 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// u = (2*(W>>12)+1) * 2^-53 with W = hi<<32 | lo: the 52 bits are OR-ed into the mantissa of 1.0;
-// subtracting 1.0 and adding 2^-53 are both exact, so no int->fp conversion is needed (reading R-3).
+// u = (2*(W>>12)+1) * 2^-53 with W = hi<<32 | lo: the 52 bits are OR-ed into the mantissa of 1.0 giving
+// 1 + m 2^-52; subtracting (1 - 2^-53) leaves (2m+1) 2^-53, which is representable, so the one DADD is exact and
+// no int->fp conversion is needed (reading R-3).
 __device__ __forceinline__ double uniform_from_words(uint32_t hi, uint32_t lo)
 {
     const double one_to_two = __hiloint2double((int)(0x3FF00000u | (hi >> 12)), (int)__funnelshift_r(lo, hi, 12));
-    return (one_to_two - 1.0) + 0x1p-53;
+    return one_to_two - (1.0 - 0x1p-53);
 }
 
 // Uniforms 2*pair and 2*pair+1 of `event`.
@@ -51,10 +52,24 @@ __device__ __forceinline__ void philox_uniform_pair(const PhiloxKey& key, uint64
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Horner helper, coefficients highest degree first.
+// Polynomial coefficients (gen_poly_coeffs.py; highest degree first) live in the constant bank: a DFMA takes them
+// as an operand (directly or through a uniform register), so no instruction is spent materialising 64-bit
+// immediates (profiles/r01a: 381 of 1848 instructions per event were such moves).
 // ---------------------------------------------------------------------------------------------------
+static __constant__ double c_PL[8] = {0x1.0c97816496c47p-3, 0x1.0fb04d4fa4e54p-3, 0x1.3b1cbf421a439p-3, 0x1.745cf674f6889p-3,
+                                      0x1.c71c72078b928p-3, 0x1.249249247343fp-2, 0x1.9999999999a4fp-2, 0x1.5555555555555p-1};
+static __constant__ double c_PE[12] = {0x1.61c2c1ba3877dp-33, 0x1.1f820dbf5e732p-29, 0x1.ae642ad2afd38p-26, 0x1.27e4d2841fc93p-22,
+                                       0x1.71de3a5af94e9p-19, 0x1.a01a01aa828e2p-16, 0x1.a01a01a0195e6p-13, 0x1.6c16c16c158f5p-10,
+                                       0x1.1111111111111p-7,  0x1.5555555555557p-5,  0x1.5555555555555p-3,  0x1.0000000000000p-1};
+// sin(pi r) = r PS(r^2), cos(pi r) = 1 + r^2 PC(r^2) on |r| <= 1/4 (max rel. error 4.9e-17 / 2.9e-17)
+static __constant__ double c_PS[8] = {-0x1.6c4a9959ac7f4p-16, 0x1.e8ee999bfa907p-12, -0x1.e3074b08b3e5dp-8, 0x1.507834859edd7p-4,
+                                      -0x1.32d2cce62aa54p-1,  0x1.466bc6775aad8p+1,  -0x1.4abbce625be53p+2, 0x1.921fb54442d18p+1};
+static __constant__ double c_PC[8] = {0x1.1e688a088894cp-18, -0x1.b6de64b9ca596p-14, 0x1.f9d386d6a8da6p-10, -0x1.a6d1f2a0675b5p-6,
+                                      0x1.e1f506891ad52p-3,  -0x1.55d3c7e3cbff7p+0,  0x1.03c1f081b5ac4p+2,  -0x1.3bd3cc9be45dep+2};
+
+// Horner, coefficients highest degree first.
 template <int NC>
-__device__ __forceinline__ double horner(const double (&c)[NC], double x)
+__device__ __forceinline__ double horner(const double* c, double x)
 {
     double r = c[0];
 #pragma unroll
@@ -63,74 +78,146 @@ __device__ __forceinline__ double horner(const double (&c)[NC], double x)
 }
 
 // ---------------------------------------------------------------------------------------------------
-// ln(y) for y in (0,1], given also z = 1 - y.  When `z_exact` (the caller obtained z without
-// cancellation and y = 1 - z), the reduced argument is taken from z for y >= sqrt(1/2), which is what
-// log1p(-z) would do -- but in the same instruction stream as the plain logarithm.
-//   y = m 2^e, m in [sqrt(1/2), sqrt(2)), f = m - 1, s = f/(2+f), ln m = f - s (f - s^2 PL(s^2)).
+// Guard-free reciprocal, square root and integer root for arguments known to be positive, normal and far from
+// the ends of the exponent range (everything on this path is): one MUFU seed (2^-22) and Newton / Halley steps
+// on the fp64 pipe, no slow-path branch.
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double log_unit(double y, double z, bool z_exact)
+__device__ __forceinline__ double rcp_fast(double a)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+    double e = fma(-a, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-a, r, 1.0);
+    return fma(r, e, r);
+}
+
+// sqrt(a); `half_rsqrt` receives 1/(2 sqrt(a)) to about 2^-43 (enough as a Newton seed or a weight factor's inverse).
+__device__ __forceinline__ double sqrt_fast(double a, double& half_rsqrt)
+{
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+    double g = a * r, h = 0.5 * r;
+    double e = fma(-g, h, 0.5);
+    g = fma(g, e, g);
+    h = fma(h, e, h);
+    e = fma(-g, h, 0.5);
+    g = fma(g, e, g);
+    h = fma(h, e, h);
+    const double d = fma(-g, g, a);
+    half_rsqrt = h;
+    return fma(d, h, g);
+}
+__device__ __forceinline__ double sqrt_fast(double a)
+{
+    double h;
+    return sqrt_fast(a, h);
+}
+
+// y^(1/R), y in (0,1], R >= 3: fp32 seed exp2(log2(y)/R) from MUFU.LG2/EX2 (relative error e ~ 2^-21), then one
+// Halley step u (R-1) u^R + (R+1) y over (R+1) u^R + (R-1) y, whose error is (R^2-1)/12 e^3 < 1e-17 for R <= 14.
+template <int R>
+__device__ __forceinline__ double root_fast(double y)
+{
+    const float yf = __double2float_rn(y);
+    float l, uf;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(yf));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(uf) : "f"(l * (1.0f / R)));
+    const double u = (double)uf;
+    double p = u;
+    if constexpr (R % 2 == 0) {
+        double q = u * u;                        // u^R = (u^2)^(R/2) by squaring
+        p = 1.0;
+#pragma unroll
+        for (int b = R / 2; b > 0; b >>= 1) {
+            if (b & 1) p *= q;
+            if (b > 1) q *= q;
+        }
+    } else {
+        double q = u;
+        p = 1.0;
+#pragma unroll
+        for (int b = R; b > 0; b >>= 1) {
+            if (b & 1) p *= q;
+            if (b > 1) q *= q;
+        }
+    }
+    const double num = fma((double)(R - 1), p, (double)(R + 1) * y);
+    const double den = fma((double)(R + 1), p, (double)(R - 1) * y);
+    return u * num * rcp_fast(den);
+}
+
+// sin(2 pi x), cos(2 pi x) for x in (0,1): quarter-turn reduction q = rint(4x), r = 2x - q/2 in [-1/4, 1/4] (exact),
+// the two cores above, then the rotation by q quarter turns as one swap and two sign flips.
+__device__ __forceinline__ void sincos_2pi(double x, double& sn, double& cs)
+{
+    const double magic = 0x1.8p52;
+    const double qm = fma(4.0, x, magic);                       // low word = q
+    const int q = __double2loint(qm);
+    const double r = fma(-0.5, qm - magic, 2.0 * x);
+    const double r2 = r * r;
+    const double s = r * horner<8>(c_PS, r2);
+    const double c = fma(r2, horner<8>(c_PC, r2), 1.0);
+    const bool odd = q & 1;
+    const double a = odd ? c : s;                               // sin(pi r + q pi/2)
+    const double b = odd ? s : c;
+    const int sa = (int)(((unsigned)q & 2u) << 30), sb = (int)(((unsigned)(q + 1) & 2u) << 30);
+    sn = __hiloint2double(__double2hiint(a) ^ sa, __double2loint(a));
+    cs = __hiloint2double(__double2hiint(b) ^ sb, __double2loint(b));
+}
+
+// ---------------------------------------------------------------------------------------------------
+// ln(y) for y in (0,1] (normal).  y = m 2^e, m in [sqrt(1/2), sqrt(2)), f = m - 1, s = f/(2+f),
+// ln m = f - s (f - s^2 PL(s^2)).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double log_unit(double y)
 {
     const int hi = __double2hiint(y), lo = __double2loint(y);
     int e = (hi >> 20) - 1023;
     int mhi = (hi & 0x000FFFFF) | 0x3FF00000;
     if (mhi >= 0x3FF6A09F) { mhi -= 0x00100000; e += 1; }
     const double m = __hiloint2double(mhi, lo);
-    double f = m - 1.0;
-    if (z_exact && e == 0) f = -z;
-    const double s = f / (2.0 + f);
+    const double f = m - 1.0;
+    const double s = f * rcp_fast(2.0 + f);
     const double z2 = s * s;
-    const double PL[8] = {0x1.0c97816496c47p-3, 0x1.0fb04d4fa4e54p-3, 0x1.3b1cbf421a439p-3, 0x1.745cf674f6889p-3,
-                          0x1.c71c72078b928p-3, 0x1.249249247343fp-2, 0x1.9999999999a4fp-2, 0x1.5555555555555p-1};
-    const double R = horner(PL, z2);
+    const double R = horner<8>(c_PL, z2);
     const double lnm = fma(-s, fma(-z2, R, f), f);
     return fma((double)e, 0x1.62e42fefa39efp-1, lnm);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// exp(h) and expm1(h) for h <= 0 from one range reduction: h = n ln2 + r, |r| <= ln2/2,
-// expm1(r) = r + r^2 PE(r);  exp(h) = 2^n (1 + p),  expm1(h) = 2^n p + (2^n - 1)  (no cancellation for n <= 0).
+// exp(h) for moderate h (|h| < 700): h = n ln2 + r, |r| <= ln2/2, expm1(r) = r + r^2 PE(r), exp(h) = 2^n (1 + p).
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void exp_expm1_neg(double h, double& ex, double& em1)
-{
-    const int n = __double2int_rn(h * 0x1.71547652b82fep+0);
-    const double nd = (double)n;
-    double r = fma(-nd, 0x1.62e42fee00000p-1, h);
-    r = fma(-nd, 0x1.a39ef35793c76p-33, r);
-    const double PE[12] = {0x1.61c2c1ba3877dp-33, 0x1.1f820dbf5e732p-29, 0x1.ae642ad2afd38p-26, 0x1.27e4d2841fc93p-22,
-                           0x1.71de3a5af94e9p-19, 0x1.a01a01aa828e2p-16, 0x1.a01a01a0195e6p-13, 0x1.6c16c16c158f5p-10,
-                           0x1.1111111111111p-7,  0x1.5555555555557p-5,  0x1.5555555555555p-3,  0x1.0000000000000p-1};
-    const double p = fma(r * r, horner(PE, r), r);
-    const double sc = __hiloint2double((n + 1023) << 20, 0);
-    ex = fma(sc, p, sc);
-    em1 = fma(sc, p, sc - 1.0);
-}
-
-// exp(h) for any moderate h (|h| < 700).
 __device__ __forceinline__ double exp_any(double h)
 {
-    double ex, em1;
-    exp_expm1_neg(h, ex, em1);   // the reduction is sign-agnostic; only em1's conditioning needs h <= 0
-    return ex;
+    const double magic = 0x1.8p52;
+    const double nm = fma(h, 0x1.71547652b82fep+0, magic);
+    const int n = __double2loint(nm);
+    const double nd = nm - magic;
+    double r = fma(-nd, 0x1.62e42fee00000p-1, h);
+    r = fma(-nd, 0x1.a39ef35793c76p-33, r);
+    const double p = fma(r * r, horner<12>(c_PE, r), r);
+    const double sc = __hiloint2double((n + 1023) << 20, 0);
+    return fma(sc, p, sc);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// G_RQF^{-1}(x; c): Eq. 65 for x <= 1/2 and the same quadratic solved for z = 1-y for
-// x > 1/2 (reading M-2), merged: with t = min-side variable, g = (c-2) t,
-//   low : beta = c - g, alpha = 1 - beta, y = 2t / (beta + sqrt(beta^2 + 4 t alpha))
-//   high: beta = g,     alpha = 1 + g,    z = (beta + sqrt(beta^2 + 4 t alpha)) / (2 alpha)
+// G_RQF^{-1}(x; c), both y and z = 1 - y, with no branch and no cancellation.  Eq. 65 is
+// y = 2x / (b + sqrt(b^2 - 4x(b-1))), b = c - (c-2)x; the same quadratic written for z (reading M-2) is
+// z = (beta + sqrt(beta^2 + 4s(1+beta))) / (2(1+beta)), s = 1-x, beta = (c-2)s.  Since b = 2 + beta the two
+// discriminants are the same number, so one square root and one reciprocal give both roots, every term positive.
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void rqf_inverse(double x, double c, double& y, double& z, bool& high)
+__device__ __forceinline__ void rqf_inverse(double x, double c, double& y, double& z)
 {
-    high = x > 0.5;
-    const double t = high ? 1.0 - x : x;
-    const double g = (c - 2.0) * t;
-    const double beta = high ? g : c - g;
-    const double alpha = high ? 1.0 + g : 1.0 - beta;
-    const double sq = sqrt(fma(beta, beta, 4.0 * t * alpha));
-    const double bs = beta + sq;
-    const double q = (high ? bs : 2.0 * t) / (high ? 2.0 * alpha : bs);
-    y = high ? 1.0 - q : q;
-    z = high ? q : 1.0 - q;
+    const double s = 1.0 - x;
+    const double beta = (c - 2.0) * s;
+    const double a = 1.0 + beta;
+    const double sq = sqrt_fast(fma(beta, beta, 4.0 * s * a));
+    const double d1 = (a + 1.0) + sq;
+    const double a2 = a + a;
+    const double inv = rcp_fast(d1 * a2);
+    y = (2.0 * x) * a2 * inv;
+    z = (beta + sq) * d1 * inv;
 }
 
 // Table 1: fitted c_k*, k = 1..7.
@@ -140,22 +227,45 @@ __device__ __forceinline__ constexpr double table1_ck(int k)
          : k == 6 ? 3.578833 : 3.662872;
 }
 
+// v = y^(1/K) and u = sqrt(v) = y^(1/(2K)) (Eq. 60), and 1 - v = z / (1 + v + ... + v^(K-1)) from
+// z = 1 - y (exact factorisation: no cancellation, no logarithm).  Returns S = 1 + v + ... + v^(K-1).
+template <int K>
+__device__ __forceinline__ double mass_ratio(double y, double z, double& u, double& omu2)
+{
+    if constexpr (K == 1) {
+        u = sqrt_fast(y);
+        omu2 = z;
+        return 1.0;
+    } else {
+        double v;
+        if constexpr (K == 2) {
+            v = sqrt_fast(y);
+            u = sqrt_fast(v);
+        } else {
+            u = root_fast<2 * K>(y);
+            v = u * u;
+        }
+        double S = 1.0 + v;
+#pragma unroll
+        for (int j = 2; j < K; ++j) S = fma(S, v, 1.0);
+        omu2 = z * rcp_fast(S);
+        return S;
+    }
+}
+
 // One FastRambo mass step (Eq. 60, 65; weight factor = Eq. 67 / Eq. 63):
-//   u = y^{1/(2k)}, omu2 = 1 - u^2 = 1 - y^{1/k}, weight factor (k+1) omu2 / g_RQF(y) = wnum / wden.
+//   weight factor (k+1)(1 - y^(1/k)) / g_RQF(y) with g_RQF = z (2y + c z) / D^2, D = 1 + (c-2) y z (Eq. 64, 1-y = z)
+//   = (k+1) D^2 / ((2y + c z) S) = wnum / wden   (the z of 1 - y^(1/k) = z/S cancels).
 template <int K>
 __device__ __forceinline__ void fastrambo_mass_step(double x, double& u, double& omu2, double& wnum, double& wden)
 {
     constexpr double c = table1_ck(K);
     double y, z;
-    bool high;
-    rqf_inverse(x, c, y, z, high);
-    const double L = log_unit(y, z, high);
-    double em1;
-    exp_expm1_neg(L * (0.5 / K), u, em1);          // u = exp(L/2k), em1 = u - 1
-    omu2 = -em1 * (1.0 + u);                       // 1 - u^2 = (1-u)(1+u)
+    rqf_inverse(x, c, y, z);
+    const double S = mass_ratio<K>(y, z, u, omu2);
     const double D = fma((c - 2.0) * y, z, 1.0);
-    wnum = (double)(K + 1) * omu2 * (D * D);       // g_RQF = z (2y + c z) / D^2   (Eq. 64 with 1-y = z)
-    wden = z * fma(c, z, 2.0 * y);
+    wnum = (double)(K + 1) * (D * D);
+    wden = fma(c, z, 2.0 * y) * S;
 }
 
 // Binomial coefficient at compile time.
@@ -177,22 +287,20 @@ template <int K>
 __device__ __forceinline__ bool rambo_mass_step(double r, double& u, double& omu2)
 {
     if constexpr (K == 1) {
-        const double t = sqrt(1.0 - r);            // (1-v)^2 = 1-r
-        const double v = r / (1.0 + t);
-        u = sqrt(v);
+        const double t = sqrt_fast(1.0 - r);       // (1-v)^2 = 1-r
+        const double v = r * rcp_fast(1.0 + t);
+        u = sqrt_fast(v);
         omu2 = t;
         return true;
     } else {
         constexpr double c = table1_ck(K);
-        double y, z;
-        bool high;
-        rqf_inverse(r, c, y, z, high);
-        const double L = log_unit(y, z, high);
-        double v0, em1;
-        exp_expm1_neg(L * (1.0 / K), v0, em1);
+        double y, z, u0, t0;
+        rqf_inverse(r, c, y, z);
+        mass_ratio<K>(y, z, u0, t0);                 // FastRambo start value: v0 = u0^2, t0 = 1 - v0
+        const bool high = r > 0.5;
         const double tgt = high ? 1.0 - r : r;
-        double w = high ? -em1 : v0;
-        if (high && tgt < 1e-3) w = sqrt(tgt * (2.0 / (K * (K + 1.0))));
+        double w = high ? t0 : u0 * u0;
+        if (high && tgt < 1e-3) w = sqrt_fast(tgt * (2.0 / (K * (K + 1.0))));
         // per-lane coefficients c_j, j = 2..K+1
         double cj[K + 2];
 #pragma unroll
@@ -213,7 +321,7 @@ __device__ __forceinline__ bool rambo_mass_step(double r, double& u, double& omu
             }
             G = G * w * w;
             H = H * w;
-            double wn = w - (G - tgt) / H;
+            double wn = w - (G - tgt) * rcp_fast(H);
             if (!(wn > 0.0)) wn = 0.5 * w;
             if (!(wn < 1.0)) wn = 0.5 * (w + 1.0);
             const double step = fabs(wn - w);
@@ -226,7 +334,7 @@ __device__ __forceinline__ bool rambo_mass_step(double r, double& u, double& omu
         if (!done) ok = false;
         const double v = high ? 1.0 - w : w;
         omu2 = high ? w : 1.0 - w;
-        u = sqrt(v);
+        u = sqrt_fast(v);
         return ok;
     }
 }
@@ -245,9 +353,9 @@ template <bool FIRST>
 __device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double q, double x_cos, double x_phi, Vec4& p)
 {
     const double cth = fma(2.0, x_cos, -1.0);
-    const double sth = 2.0 * sqrt(x_cos * (1.0 - x_cos));   // sqrt(1 - cth^2) without cancellation
+    const double sth = 2.0 * sqrt_fast(x_cos * (1.0 - x_cos));   // sqrt(1 - cth^2) without cancellation
     double sn, cs;
-    sincospi(2.0 * x_phi, &sn, &cs);
+    sincos_2pi(x_phi, sn, cs);
     const double qs = q * sth;
     const double rx = qs * cs, ry = qs * sn, rz = q * cth;
     if constexpr (FIRST) {
@@ -255,7 +363,7 @@ __device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double q, doub
         Q.e = M - q; Q.x = -rx; Q.y = -ry; Q.z = -rz;
     } else {
         const double qm = Q.e + M;
-        const double inv = 1.0 / (M * qm);
+        const double inv = rcp_fast(M * qm);
         const double ep = fma(Q.x, rx, fma(Q.y, ry, fma(Q.z, rz, Q.e * q))) * (inv * qm);
         const double f = (q + ep) * (inv * M);
         p.e = ep;

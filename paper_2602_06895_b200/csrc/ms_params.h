@@ -28,6 +28,8 @@ struct GenParams {
     double phi_unit;           // Phi_n(1), Eq. 81
     double phi_fixed;          // Phi_n(sqrt_s) when the energy is fixed
     double ln_tau_min, rel_tol, toy_reg;
+    double grid_bins_f;        // (double)grid_bins
+    double jac_scale;          // grid_bins^grid_dims: the VEGAS Jacobian is jac_scale * prod of bin widths
     double masses[kMaxN];
     double* p;                 // [4(n+2)][ld]
     double* w;                 // [N]
