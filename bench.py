@@ -31,27 +31,62 @@ METRIC = "phase-space events/s (fp64, weighted events through the whole hot path
 UNIT = "events/s"
 FP64_LANES_PER_SM = 64            # B200 (GB100): 64 FP64 FMA lanes per SM (datasheet 37 TFLOP/s = 148*64*2*1.965 GHz)
 
-# Hand-counted fp64-pipe instructions of the final formulas: per stage.
-ALG_FP64 = {"vegas_dim": 6, "fast_mass": 96, "exact_mass_k1": 40, "exact_mass": 150, "decay": 64, "decay_first": 44,
-            "toy_pair": 15, "toy_particle": 11, "weight": 14, "pdf": 75, "boost_particle": 4,
-            "rescale_iter_massive": 16, "rescale_iter_massless": 2, "rescale_fixed": 40}
+# Hand-counted fp64-pipe instructions (DADD/DMUL/DFMA/DSETP) of the final formulas, per stage (DESIGN.md §5
+# "algorithmic op count"; MUFU seeds and int<->fp conversions run on the XU pipe and are not counted here).
+RCP, SQRT = 4, 10          # Newton steps after the MUFU seed: rcp_fast, sqrt_fast (with the 1/(2 sqrt) by-product)
+RQF_INVERSE = 29           # s, beta, a, discriminant (4), sqrt, d1 (2), a2, product, rcp, y (3), z (3)
+EXP = 18                   # magic-number reduction (4), r^2, degree-11 Horner, 2 fma
+SINCOS = 21                # quarter-turn reduction (4), r^2, two degree-7 Horners, 2
+
+
+def _pow_cost(r):          # multiplications of u^r by squaring
+    return max(r.bit_length() - 1 + bin(r).count("1") - 1, 0)
+
+
+def _mass_ratio(k):        # v = y^(1/k), u = sqrt(v), 1 - v = z / (1 + v + ... + v^(k-1))
+    if k == 1:
+        return SQRT - 1
+    if k == 2:
+        return 2 * (SQRT - 1) + 1 + RCP + 1
+    return _pow_cost(2 * k) + 4 + RCP + 2 + 1 + (k - 1) + RCP + 1      # Halley root of order 2k, v, S, rcp, 1-v
+
+
+def fast_mass_step(k):     # RQF inverse, ratio, weight factor (k+1) D^2 / ((2y + c z) S), q, M, weight products
+    return RQF_INVERSE + _mass_ratio(k) + (3 if k == 1 else 7) + 5
+
+
+def exact_mass_step(k, newton_iterations=4):
+    if k == 1:
+        return 1 + SQRT - 1 + 1 + RCP + 1 + SQRT - 1 + 3
+    per_iter = 2 * k + 3 + 1 + RCP + 1 + 5                              # two Horners, residual, rcp, update, guards
+    return RQF_INVERSE + _mass_ratio(k) + newton_iterations * per_iter + 4 + SQRT - 1 + 3
+
+
+ALG_FP64 = {"uniform": 1, "vegas_dim": 5, "decay_first": 3 + SQRT - 1 + 1 + SINCOS + 4 + 1,
+            "decay": 3 + SQRT - 1 + 1 + SINCOS + 4 + 2 + RCP + 4 + 4 + 3 + 4,
+            "toy_pair": 13, "weight": 5 + RCP + 3 + 3, "pdf": 2 * EXP + 4 + RCP + 2 + 4 + 3 + 4, "boost_particle": 4,
+            "rescale_start": 1 + RCP + 1 + 1 + SQRT - 1, "rescale_eval_massive": 2 + SQRT + 4, "rescale_eval_massless": 2,
+            "rescale_eval_fixed": 2 + RCP + 1, "rescale_final_massive": 2 + SQRT + 4 + 3, "rescale_final_massless": 5,
+            "rescale_weight": 3 + 3 + RCP}
+RESCALE_EVALUATIONS = 4    # cfg4 converges in <= 3 Newton steps: 4 evaluations of F
 
 
 def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
     n = wl.n
-    c = ALG_FP64["vegas_dim"] * wl.grid_dims
-    if wl.mapping == "fastrambo":
-        c += ALG_FP64["fast_mass"] * (n - 2)
-    else:
-        c += ALG_FP64["exact_mass"] * max(n - 3, 0) + (ALG_FP64["exact_mass_k1"] if n > 2 else 0)
+    c = ALG_FP64["uniform"] * wl.d + ALG_FP64["vegas_dim"] * wl.grid_dims
+    for i in range(2, n):
+        c += fast_mass_step(n - i) if wl.mapping == "fastrambo" else exact_mass_step(n - i)
     c += ALG_FP64["decay_first"] + ALG_FP64["decay"] * (n - 2)
     if wl.toy:
-        c += ALG_FP64["toy_particle"] * n + ALG_FP64["toy_pair"] * (n - 1)
+        c += ALG_FP64["toy_pair"] * (n - 1)
     if wl.pdf:
         c += ALG_FP64["pdf"] + ALG_FP64["boost_particle"] * n
     if wl.masses:
         nm = sum(1 for m in wl.masses if m > 0)
-        c += ALG_FP64["rescale_fixed"] + 4 * (ALG_FP64["rescale_iter_massive"] * nm + ALG_FP64["rescale_iter_massless"] * (n - nm) + 12)
+        c += ALG_FP64["rescale_start"] + ALG_FP64["rescale_weight"]
+        c += RESCALE_EVALUATIONS * (ALG_FP64["rescale_eval_massive"] * nm + ALG_FP64["rescale_eval_massless"] * (n - nm)
+                                    + ALG_FP64["rescale_eval_fixed"])
+        c += ALG_FP64["rescale_final_massive"] * nm + ALG_FP64["rescale_final_massless"] * (n - nm)
     return c + ALG_FP64["weight"]
 
 
@@ -75,7 +110,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             pass
@@ -241,21 +276,24 @@ def run_ours(args):
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    gen_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stages = [("generate", lambda: hp.generate(offset))]
+    if wl.unweight:
+        stages.append(("unweight", lambda: hp.unweight(offset)))
+    if wl.inverse:
+        stages.append(("fastrambo_inverse", hp.invert_phase_space))
+        stages.append(("vegas_inverse", hp.invert_grid))
+    marks = [[torch.cuda.Event(enable_timing=True) for _ in range(len(stages) + 1)] for _ in range(args.steps)]
     ev[0].record(stream)
     for k in range(args.steps):
-        gen_ev[k][0].record(stream)
-        hp.generate(offset)
-        gen_ev[k][1].record(stream)
-        if wl.unweight:
-            hp.unweight(offset)
-        if wl.inverse:
-            hp.invert()
+        marks[k][0].record(stream)
+        for j, (_, fn) in enumerate(stages):
+            fn()
+            marks[k][j + 1].record(stream)
     ev[1].record(stream)
     barrier()
-    clocks = sampler.stop() if sampler else None
     t_total = ev[0].elapsed_time(ev[1]) * 1e-3
-    t_gen = float(np.mean([a.elapsed_time(b) for a, b in gen_ev])) * 1e-3
+    stage_ms = {name: float(np.mean([m[j].elapsed_time(m[j + 1]) for m in marks])) for j, (name, _) in enumerate(stages)}
+    t_gen = stage_ms["generate"] * 1e-3
     n_acc_local = int(hp.n_acc.item()) if wl.unweight else 0
     if world > 1:
         tt = torch.tensor([t_total, t_gen], dtype=torch.float64, device=dev)
@@ -294,6 +332,7 @@ def run_ours(args):
         e2e_step()
     ev[1].record(stream)
     barrier()
+    clocks = sampler.stop() if sampler else None          # sampled over both timed regions (device-resident and e2e)
     t_e2e = max(ev[0].elapsed_time(ev[1]) * 1e-3, 0.0)
     t_e2e_wall = time.perf_counter() - t0
     if world > 1:
@@ -339,7 +378,7 @@ def run_ours(args):
                     "what": "grid table H2D from pinned memory + whole step + D2H of %s, host waits every step"
                             % ("the accepted count and the compacted unweighted sample (idx, w_out, momentum rows; cap %d)" % hp.cap
                                if wl.unweight else "all momenta and weights")},
-            "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "cpu_baseline": cb,
+            "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "stage_ms": stage_ms, "cpu_baseline": cb,
             "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
                             "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
             "fail_count": int(hp.fail.item()),
@@ -353,7 +392,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg2", choices=sorted(ms_inputs.WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])

@@ -70,8 +70,9 @@ int ms_check_grid(int d, int n_bins, const double* h_edges);
  *   direction 0 (forward):  t = r*n_bins, j = min(floor t, n_bins-1), x = x_j + (t-j)(x_{j+1}-x_j),
  *       clamped into [2^-53, 1-2^-53]; d_jac[e] = prod_dims n_bins (x_{j+1}-x_j).
  *       d_in = r rows [d][ld], or NULL -> Philox uniforms j = 0..d-1 of stream rng.stream.
- *   direction 1 (inverse):  j = bin with x_j <= x < x_{j+1} (per-lane binary search over the
- *       shared-memory edge table), r = (j + (x-x_j)/(x_{j+1}-x_j))/n_bins; d_jac[e] = 1/prod(...).
+ *   direction 1 (inverse):  j = bin with x_j <= x < x_{j+1} (binary search, every lane of a warp descending its
+ *       own path through a breadth-first edge tree in shared memory), r = (j + (x-x_j)/(x_{j+1}-x_j))/n_bins;
+ *       d_jac[e] = 1/prod(...).
  *       d_in = x rows (must not be NULL).
  * d_edges: device table [d][n_bins+1], validated by the caller with ms_check_grid.
  * d_out: [d][ld].  d_jac: [N] or NULL.  d_in and d_out may alias. */
@@ -132,13 +133,14 @@ int ms_toy_integrand(int64_t N, int n, double reg, const double* d_p, double* d_
 int ms_reduce_max(int64_t N, const double* d_w, double* d_out, void* stream);
 
 /* ms_unweight -- single-pass hit-or-miss unweighting against a fixed w_max (reading U)
- * with stable stream compaction (warp ballot + block scan + decoupled look-back across tiles).
+ * with stable stream compaction (warp ballots per 512-event tile, one scan of the tile counts, scatter of the
+ * accepted events: three kernels on `stream`, none of which waits on another's progress).
  *   accept_e <=> u_e * w_max < w_e, u_e = Philox uniform j=0 of (rng.seed, rng.stream, event);
  *   accepted events are written in increasing event order: d_idx[k] = e, d_w_out[k] = max(1, w_e/w_max),
  *   d_rows_out[r*cap + k] = d_rows_in[r*ld + e] for r < n_rows (skipped if either pointer is NULL).
  *   *d_n_accepted = true number accepted; only the first `cap` are stored.
- * d_wmax: device scalar.  d_scratch: ms_unweight_scratch_bytes(N) bytes, any content (the call
- * clears it on the stream). */
+ * d_wmax: device scalar.  d_scratch: ms_unweight_scratch_bytes(N) bytes (72 B per 512 events), any content, 16-byte
+ * aligned; overwritten. */
 size_t ms_unweight_scratch_bytes(int64_t N);
 int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, int n_rows, const double* d_rows_in,
                 int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted,

@@ -98,3 +98,27 @@ def main():
 
 if __name__ == "__main__":
     main()
+
+
+def atan_turns():
+    """atan(t) / (2 pi) = t * PA(t^2) on |t| <= sqrt(2) - 1 (the FastRambo inverse's azimuth, in turns)."""
+    zmax = (mp.sqrt(2) - 1) ** 2 * mp.mpf("1.01")
+
+    def g(z):
+        if z < mp.mpf(10) ** -30:
+            return 1 / (2 * mp.pi)
+        t = mp.sqrt(z)
+        return mp.atan(t) / (2 * mp.pi * t)
+
+    pa = fit(g, 0, zmax, 12)
+    show("PA", pa)
+    worst = 0
+    for i in range(1, 3001):
+        t = (mp.sqrt(2) - 1) * i / 3000
+        ap = t * mp.polyval([mp.mpf(float(c)) for c in pa], t * t)
+        worst = max(worst, abs(ap / (mp.atan(t) / (2 * mp.pi)) - 1))
+    print("// atan (turns) core max rel err", mp.nstr(worst, 5))
+
+
+if __name__ == "__main__":
+    atan_turns()

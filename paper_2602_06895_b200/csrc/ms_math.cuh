@@ -67,6 +67,11 @@ static __constant__ double c_PS[8] = {-0x1.6c4a9959ac7f4p-16, 0x1.e8ee999bfa907p
 static __constant__ double c_PC[8] = {0x1.1e688a088894cp-18, -0x1.b6de64b9ca596p-14, 0x1.f9d386d6a8da6p-10, -0x1.a6d1f2a0675b5p-6,
                                       0x1.e1f506891ad52p-3,  -0x1.55d3c7e3cbff7p+0,  0x1.03c1f081b5ac4p+2,  -0x1.3bd3cc9be45dep+2};
 
+// atan(t) / (2 pi) = t PA(t^2) on |t| <= sqrt(2) - 1 (max rel. error 6.6e-17)
+static __constant__ double c_PA[12] = {-0x1.7051651483447p-9, 0x1.8a943f5548953p-8, -0x1.065065cdaaeecp-7, 0x1.30dd6cc651060p-7,
+                                       -0x1.5b7a2c88f6247p-7, 0x1.91276be34fb19p-7, -0x1.da1b804092706p-7, 0x1.21bb93a648421p-6,
+                                       -0x1.7483758b589b1p-6, 0x1.04c26be3acccdp-5, -0x1.b2995e7b7b5cep-5, 0x1.45f306dc9c883p-3};
+
 // Horner, coefficients highest degree first.
 template <int NC>
 __device__ __forceinline__ double horner(const double* c, double x)
@@ -92,7 +97,7 @@ __device__ __forceinline__ double rcp_fast(double a)
     return fma(r, e, r);
 }
 
-// sqrt(a); `half_rsqrt` receives 1/(2 sqrt(a)) to about 2^-43 (enough as a Newton seed or a weight factor's inverse).
+// sqrt(a) to 1 ulp; `half_rsqrt` receives 1/(2 sqrt(a)) from the same two Newton steps (a few ulp).
 __device__ __forceinline__ double sqrt_fast(double a, double& half_rsqrt)
 {
     double r;
@@ -164,6 +169,25 @@ __device__ __forceinline__ void sincos_2pi(double x, double& sn, double& cs)
     const int sa = (int)(((unsigned)q & 2u) << 30), sb = (int)(((unsigned)(q + 1) & 2u) << 30);
     sn = __hiloint2double(__double2hiint(a) ^ sa, __double2loint(a));
     cs = __hiloint2double(__double2hiint(b) ^ sb, __double2loint(b));
+}
+
+// atan2(y, x) / (2 pi) folded into [0, 1) (the azimuth uniform of Eq. 25 inverted, reading F-4): first octant
+// a = min/max in [0,1]; for a > tan(pi/8) the argument is reduced by atan a = pi/4 + atan((a-1)/(a+1)), which with
+// a = mn/mx is (mn-mx)/(mn+mx), so ONE reciprocal serves both cases; then the octant is unfolded by three reflections.
+__device__ __forceinline__ double atan2_turns(double y, double x)
+{
+    const double ax = fabs(x), ay = fabs(y);
+    const bool swap = ay > ax;
+    const double mx = swap ? ay : ax, mn = swap ? ax : ay;
+    const bool big = mn > 0x1.a827999fcef32p-2 * mx;            // tan(pi/8)
+    const double num = big ? mn - mx : mn;
+    const double den = big ? mn + mx : mx;
+    const double t = num * rcp_fast(den);
+    double turn = fma(t, horner<12>(c_PA, t * t), big ? 0.125 : 0.0);
+    if (swap) turn = 0.25 - turn;
+    if (x < 0.0) turn = 0.5 - turn;
+    if (y < 0.0) turn = 1.0 - turn;
+    return turn;
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -102,13 +102,18 @@ class HotPath:
                     self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
                     self.scratch, self.scratch_bytes, self.ld, stream)
 
-    def invert(self, stream=None) -> None:
-        s = self.spec
-        ms_fastrambo_inverse(self.N, s.n, self.p, self.x_inv, self.w_inv, self.ld, stream)
+    def invert_phase_space(self, stream=None) -> None:
+        ms_fastrambo_inverse(self.N, self.spec.n, self.p, self.x_inv, self.w_inv, self.ld, stream)
+
+    def invert_grid(self, stream=None) -> None:
         if self.d_edges is not None:
             # only the dimensions the phase-space map consumed are inverted
             ms_vegas_map(self.N, self.d_inv, self.grid_bins, self.d_edges, 1, self.x_inv, rng(0), self.r_inv, None,
                          self.ld, stream)
+
+    def invert(self, stream=None) -> None:
+        self.invert_phase_space(stream)
+        self.invert_grid(stream)
 
     def step(self, event_offset: int = 0, stream=None) -> None:
         self.generate(event_offset, stream)
@@ -122,7 +127,7 @@ class HotPath:
         """Kernels of this library enqueued by one step() (memsets/copies not counted)."""
         k = 1
         if self.spec.unweight:
-            k += 2
+            k += 4                                  # ms_reduce_max + decide / scan / scatter of ms_unweight
         if self.spec.inverse:
             k += 2 if self.d_edges is not None else 1
         return k

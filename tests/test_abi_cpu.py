@@ -103,5 +103,5 @@ def test_empty_batches_are_no_ops(ms):
 
 def test_scratch_size(ms):
     assert ms.ms_unweight_scratch_bytes(0) == 256
-    assert ms.ms_unweight_scratch_bytes(1 << 24) >= 8 * ((1 << 24) // 1024 + 1)
+    assert ms.ms_unweight_scratch_bytes(1 << 24) >= 8 * ((1 << 24) // 512 + 1)
     assert ms.ms_unweight_scratch_bytes(1 << 24) % 256 == 0
