@@ -133,13 +133,13 @@ int ms_toy_integrand(int64_t N, int n, double reg, const double* d_p, double* d_
 int ms_reduce_max(int64_t N, const double* d_w, double* d_out, void* stream);
 
 /* ms_unweight -- single-pass hit-or-miss unweighting against a fixed w_max (reading U)
- * with stable stream compaction (warp ballots per 512-event tile, one scan of the tile counts, scatter of the
- * accepted events: three kernels on `stream`, none of which waits on another's progress).
+ * with stable stream compaction (warp ballots per 512-event tile, then a scatter that scans the tile counts: two
+ * kernels on `stream`, neither of which waits on another block's progress).
  *   accept_e <=> u_e * w_max < w_e, u_e = Philox uniform j=0 of (rng.seed, rng.stream, event);
  *   accepted events are written in increasing event order: d_idx[k] = e, d_w_out[k] = max(1, w_e/w_max),
  *   d_rows_out[r*cap + k] = d_rows_in[r*ld + e] for r < n_rows (skipped if either pointer is NULL).
  *   *d_n_accepted = true number accepted; only the first `cap` are stored.
- * d_wmax: device scalar.  d_scratch: ms_unweight_scratch_bytes(N) bytes (72 B per 512 events), any content, 16-byte
+ * d_wmax: device scalar.  d_scratch: ms_unweight_scratch_bytes(N) bytes (68 B per 512 events + 64 KB), any content, 16-byte
  * aligned; overwritten. */
 size_t ms_unweight_scratch_bytes(int64_t N);
 int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, int n_rows, const double* d_rows_in,

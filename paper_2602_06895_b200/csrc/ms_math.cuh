@@ -51,6 +51,23 @@ __device__ __forceinline__ void philox_uniform_pair(const PhiloxKey& key, uint64
     b = uniform_from_words(w[2], w[3]);
 }
 
+// Clamp of a non-negative double into [2^-53, 1 - 2^-53] on its bit pattern (non-negative doubles order like
+// their high words): same result as fmin(fmax(x, 2^-53), 1 - 2^-53) for 0 <= x <= 1 at half the instructions.
+__device__ __forceinline__ double clamp_open_unit(double x)
+{
+    const int hi = __double2hiint(x), lo = __double2loint(x);
+    const int chi = min(max(hi, 0x3CA00000), 0x3FEFFFFF);
+    const int clo = hi >= 0x3FF00000 ? -1 : (hi < 0x3CA00000 ? 0 : lo);
+    return __hiloint2double(chi, clo);
+}
+
+__device__ __forceinline__ double2 lds_double2(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Polynomial coefficients (gen_poly_coeffs.py; highest degree first) live in the constant bank: a DFMA takes them
 // as an operand (directly or through a uniform register), so no instruction is spent materialising 64-bit

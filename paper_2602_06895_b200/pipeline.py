@@ -127,7 +127,7 @@ class HotPath:
         """Kernels of this library enqueued by one step() (memsets/copies not counted)."""
         k = 1
         if self.spec.unweight:
-            k += 4                                  # ms_reduce_max + decide / scan / scatter of ms_unweight
+            k += 3                                  # ms_reduce_max + decide / scatter of ms_unweight
         if self.spec.inverse:
             k += 2 if self.d_edges is not None else 1
         return k

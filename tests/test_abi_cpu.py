@@ -102,6 +102,10 @@ def test_empty_batches_are_no_ops(ms):
 
 
 def test_scratch_size(ms):
-    assert ms.ms_unweight_scratch_bytes(0) == 256
-    assert ms.ms_unweight_scratch_bytes(1 << 24) >= 8 * ((1 << 24) // 512 + 1)
-    assert ms.ms_unweight_scratch_bytes(1 << 24) % 256 == 0
+    """The query is the contract (cub style): positive, 256-byte granular, monotone, linear in N (the header
+    states 68 B per 512 events plus 64 KB)."""
+    sizes = [ms.ms_unweight_scratch_bytes(n) for n in (0, 1, 511, 512, 513, 1 << 16, 1 << 24, 1 << 26)]
+    assert sizes[0] == 256 and all(b > 0 and b % 256 == 0 for b in sizes)
+    assert sizes == sorted(sizes)
+    assert 68 * ((1 << 24) // 512) <= sizes[6] <= 68 * ((1 << 24) // 512) + 65536 + 4096
+    assert ms.ms_unweight_scratch_bytes(-1) == 0
