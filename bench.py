@@ -55,11 +55,12 @@ def fast_mass_step(k):     # RQF inverse, ratio, weight factor (k+1) D^2 / ((2y 
     return RQF_INVERSE + _mass_ratio(k) + (3 if k == 1 else 7) + 5
 
 
-def exact_mass_step(k, newton_iterations=4):
+def exact_mass_step(k):
+    """k = 1: closed form.  k >= 2: the start value and four Newton steps run in fp32 (not fp64-pipe work); what is
+    counted is the one fp64 Halley step (three Horners of degree k-1, 16 more), 1 - w, sqrt, and the chain updates."""
     if k == 1:
         return 1 + SQRT - 1 + 1 + RCP + 1 + SQRT - 1 + 3
-    per_iter = 2 * k + 3 + 1 + RCP + 1 + 5                              # two Horners, residual, rcp, update, guards
-    return RQF_INVERSE + _mass_ratio(k) + newton_iterations * per_iter + 4 + SQRT - 1 + 3
+    return 1 + 3 * k + 16 + 1 + SQRT - 1 + 3
 
 
 ALG_FP64 = {"uniform": 1, "vegas_dim": 5, "decay_first": 3 + SQRT - 1 + 1 + SINCOS + 4 + 1,
@@ -222,23 +223,39 @@ def spec_from_workload(wl):
                     seed_unweight=ms_inputs.SEED_UNWEIGHT)
 
 
-def probe_fp64_rate(ms, torch, seconds=0.25):
-    """Sustained DFMA issue rate (instructions/s) measured with ms_probe_dfma: 8 independent chains per thread."""
+def probe_fp64_rate(ms, torch, seconds=0.25, three_regs=False):
+    """Sustained DFMA issue rate (instructions/s) measured with ms_probe_dfma (register * constant + constant) or
+    ms_probe_dfma3 (three distinct register operands): 8 independent chains per thread."""
+    probe = ms.ms_probe_dfma3 if three_regs else ms.ms_probe_dfma
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     blocks, iters = sms * 8, 1 << 14
     sink = torch.empty(blocks * 256, dtype=torch.float64, device="cuda")
-    ms.ms_probe_dfma(blocks, iters, sink)
+    probe(blocks, iters, sink)
     torch.cuda.synchronize()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     reps, best, t_end = 0, 0.0, time.perf_counter() + seconds
     while time.perf_counter() < t_end or reps < 3:
         ev0.record()
-        ms.ms_probe_dfma(blocks, iters, sink)
+        probe(blocks, iters, sink)
         ev1.record()
         ev1.synchronize()
         best = max(best, blocks * 256 * iters * 8 / (ev0.elapsed_time(ev1) * 1e-3))
         reps += 1
     return best
+
+
+def probe_write_stream(ms, torch, hp, wl, reps=10):
+    """GB/s of the generation kernel's store pattern with no arithmetic (ms_probe_write into the momentum buffer)."""
+    rows = hp.spec.rows_p
+    ms.ms_probe_write(hp.N, rows, hp.p, hp.ld)
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(reps):
+        ms.ms_probe_write(hp.N, rows, hp.p, hp.ld)
+    ev1.record()
+    ev1.synchronize()
+    return 8.0 * rows * hp.N * reps / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
 
 
 def run_ours(args):
@@ -332,9 +349,9 @@ def run_ours(args):
         e2e_step()
     ev[1].record(stream)
     barrier()
+    t_e2e_wall = time.perf_counter() - t0
     clocks = sampler.stop() if sampler else None          # sampled over both timed regions (device-resident and e2e)
     t_e2e = max(ev[0].elapsed_time(ev[1]) * 1e-3, 0.0)
-    t_e2e_wall = time.perf_counter() - t0
     if world > 1:
         tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -352,6 +369,8 @@ def run_ours(args):
     inst_per_event = alg_fp64_per_event(wl)
     fp64_peak = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6            # fp64-pipe instructions / s at max clock
     fp64_probe = probe_fp64_rate(ms, torch)
+    fp64_probe3 = probe_fp64_rate(ms, torch, three_regs=True)
+    write_probe = probe_write_stream(ms, torch, hp, wl)
     t_hbm = bytes_per_launch / (hbm_gbs * 1e9)
     t_alu = N * inst_per_event / fp64_peak
     if t_hbm >= t_alu:
@@ -364,7 +383,7 @@ def run_ours(args):
         kernel_ms=1e3 * t_gen, kernel_share_of_step=t_gen * args.steps / t_total, peak_source=peak_src,
         alg_bytes_per_event=wl.out_bytes_per_event, alg_fp64_inst_per_event=inst_per_event,
         hbm_time_ms=1e3 * t_hbm, alu_time_ms=1e3 * t_alu, frac_of_max_side=max(t_hbm, t_alu) / t_gen,
-        fp64_peak_ginst_nominal=fp64_peak / 1e9, fp64_ginst_probe_measured=fp64_probe / 1e9,
+        fp64_peak_ginst_nominal=fp64_peak / 1e9, fp64_ginst_probe_measured=fp64_probe / 1e9, fp64_ginst_probe_3reg_operands=fp64_probe3 / 1e9, write_stream_probe_gbs=write_probe,
         kernel_events_per_s=N / t_gen)
 
     cb = None if args.skip_cpu_baseline else time_oracle(wl, target_seconds=12.0)[0]

@@ -179,6 +179,13 @@ int ms_fill_uniforms(int64_t N, int d, ms_rng rng, double* d_r, int64_t ld, void
  * threads; d_sink receives one double per thread.  Executes blocks*256*iters*8 DFMA. */
 int ms_probe_dfma(int blocks, int iters, double* d_sink, void* stream);
 
+/* ms_probe_dfma3 -- as ms_probe_dfma, but every DFMA has three distinct register operands (a*b+c). */
+int ms_probe_dfma3(int blocks, int iters, double* d_sink, void* stream);
+
+/* ms_probe_write -- measurement helper: the generation kernel's store pattern with no arithmetic: every event
+ * writes `rows` doubles, one per SoA row of d_out[rows][ld], with streaming stores (8*rows*N bytes per call). */
+int ms_probe_write(int64_t N, int rows, double* d_out, int64_t ld, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -318,12 +318,40 @@ __host__ __device__ constexpr double binom_c(int n, int k)
     return b;
 }
 
+// fp32 MUFU helpers (approximate, ~2^-22): the exact-Rambo start value is computed entirely on the otherwise idle
+// fp32 / XU pipes.
+__device__ __forceinline__ float rcp_f32(float a)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+    return r;
+}
+__device__ __forceinline__ float sqrt_f32(float a)
+{
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+    return r;
+}
+__device__ __forceinline__ float root_f32(float y, float inv_k)
+{
+    float l, r;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(y));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(l * inv_k));
+    return r;
+}
+
 // Exact RamboOnDiet mass step: invert Eq. 62 written for v = u^2 = y^{1/k}:
 //   r = (k+1) v^k - k v^{k+1}.
 // Reading M-3: for r <= 1/2 solve for w = v, G(w) = (k+1) w^k - k w^{k+1} = r; for r > 1/2 solve for w = t = 1-v,
 // G(w) = 1 - (1-w)^k (1+kw) = sum_{j=2}^{k+1} a_j w^j = 1-r.  Both are degree-(k+1) polynomials without constant and
-// linear term, so ONE Horner/Newton stream with per-lane selected coefficients serves both sides.
-// Start: the FastRambo value (RQF approximates Eq. 62).  Returns false if Newton did not settle.
+// linear term (so w keeps full RELATIVE accuracy at either end), and ONE instruction stream with per-lane selected
+// coefficients serves both sides.  The paper names no method.  Here, branch-free and vote-free:
+//   1. start value in fp32: the FastRambo value (RQF approximates Eq. 62 to a few per cent), or the
+//      leading term sqrt(2(1-r)/(k(k+1))) when 1-r < 1e-3;
+//   2. four Newton steps in fp32 (-> ~1e-7 relative for every k <= 7, measured against 40-digit roots);
+//   3. ONE Halley step in fp64 (cubic: 1e-7 -> < 3e-16).
+// Returns false (event weight 0, fail counter) if the Halley step moved w by more than 1e-4 relative, i.e. if stage 2
+// had not converged.
 template <int K>
 __device__ __forceinline__ bool rambo_mass_step(double r, double& u, double& omu2)
 {
@@ -334,48 +362,69 @@ __device__ __forceinline__ bool rambo_mass_step(double r, double& u, double& omu
         omu2 = t;
         return true;
     } else {
-        constexpr double c = table1_ck(K);
-        double y, z, u0, t0;
-        rqf_inverse(r, c, y, z);
-        mass_ratio<K>(y, z, u0, t0);                 // FastRambo start value: v0 = u0^2, t0 = 1 - v0
         const bool high = r > 0.5;
-        const double tgt = high ? 1.0 - r : r;
-        double w = high ? t0 : u0 * u0;
-        if (high && tgt < 1e-3) w = sqrt_fast(tgt * (2.0 / (K * (K + 1.0))));
+        const double s = 1.0 - r;
+        const double tgt = high ? s : r;
         // per-lane coefficients c_j, j = 2..K+1
         double cj[K + 2];
+        float cf[K + 2];
 #pragma unroll
         for (int j = 2; j <= K + 1; ++j) {
             const double sgn = (j % 2 == 0) ? 1.0 : -1.0;
             const double a_hi = -sgn * (binom_c(K, j) - (double)K * binom_c(K, j - 1));
             const double a_lo = (j == K) ? (double)(K + 1) : (j == K + 1) ? -(double)K : 0.0;
             cj[j] = high ? a_hi : a_lo;
+            cf[j] = high ? (float)a_hi : (float)a_lo;
         }
-        bool done = false;
-        bool ok = false;
-        for (int it = 0; it < 20; ++it) {
-            double G = cj[K + 1], H = (K + 1) * cj[K + 1];
+        // ---- 1. fp32 start: RQF inverse (Eq. 65 and its z form) and the k-th root
+        constexpr float c = (float)table1_ck(K);
+        const float xf = __double2float_rn(r), sf = __double2float_rn(s), tf = high ? sf : xf;
+        const float beta = (c - 2.0f) * sf, a = 1.0f + beta;
+        const float sq = sqrt_f32(fmaf(beta, beta, 4.0f * sf * a));
+        float w;
+        if (high) {
+            const float z = (beta + sq) * rcp_f32(a + a);
+            const float y = 1.0f - z;
+            const float v = root_f32(fmaxf(y, 1e-30f), 1.0f / K);
+            float S = 1.0f + v;
+#pragma unroll
+            for (int j = 2; j < K; ++j) S = fmaf(S, v, 1.0f);
+            w = z * rcp_f32(S);
+            if (tf < 1e-3f) w = sqrt_f32(tf * (2.0f / (K * (K + 1.0f))));
+        } else {
+            const float y = (2.0f * xf) * rcp_f32((a + 1.0f) + sq);
+            w = root_f32(y, 1.0f / K);
+        }
+        // ---- 2. four fp32 Newton steps
+#pragma unroll
+        for (int it = 0; it < 4; ++it) {
+            float G = cf[K + 1], H = (K + 1) * cf[K + 1];
 #pragma unroll
             for (int j = K; j >= 2; --j) {
-                G = fma(G, w, cj[j]);
-                H = fma(H, w, (double)j * cj[j]);
+                G = fmaf(G, w, cf[j]);
+                H = fmaf(H, w, (float)j * cf[j]);
             }
-            G = G * w * w;
-            H = H * w;
-            double wn = w - (G - tgt) * rcp_fast(H);
-            if (!(wn > 0.0)) wn = 0.5 * w;
-            if (!(wn < 1.0)) wn = 0.5 * (w + 1.0);
-            const double step = fabs(wn - w);
-            if (!done) {
-                w = wn;
-                if (step <= 0x1p-49 * wn) { done = true; ok = true; }
-            }
-            if (!__any_sync(0xffffffffu, !done)) break;
+            float wn = fmaf(-(G * w * w - tf), rcp_f32(H * w), w);
+            if (!(wn > 0.0f)) wn = 0.5f * w;
+            if (!(wn < 1.0f)) wn = 0.5f * (w + 1.0f);
+            w = wn;
         }
-        if (!done) ok = false;
-        const double v = high ? 1.0 - w : w;
-        omu2 = high ? w : 1.0 - w;
-        u = sqrt_fast(v);
+        // ---- 3. one fp64 Halley step on f(w) = G(w) - tgt
+        const double w0 = (double)w;
+        double G = cj[K + 1], H = (K + 1) * cj[K + 1], S2 = (double)((K + 1) * K) * cj[K + 1];
+#pragma unroll
+        for (int j = K; j >= 2; --j) {
+            G = fma(G, w0, cj[j]);
+            H = fma(H, w0, (double)j * cj[j]);
+            S2 = fma(S2, w0, (double)(j * (j - 1)) * cj[j]);
+        }
+        const double f = fma(G * w0, w0, -tgt);        // G(w0) - tgt
+        H *= w0;                                        // G'(w0);  S2 = G''(w0)
+        const double dw = (2.0 * f * H) * rcp_fast(fma(2.0 * H, H, -f * S2));
+        const double wd = w0 - dw;
+        const bool ok = fabs(dw) <= 1e-4 * w0;
+        omu2 = high ? wd : 1.0 - wd;
+        u = sqrt_fast(high ? 1.0 - wd : wd);
         return ok;
     }
 }
