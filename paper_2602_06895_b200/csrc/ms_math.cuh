@@ -101,34 +101,32 @@ __device__ __forceinline__ double horner(const double* c, double x)
 
 // ---------------------------------------------------------------------------------------------------
 // Guard-free reciprocal, square root and integer root for arguments known to be positive, normal and far from
-// the ends of the exponent range (everything on this path is): one MUFU seed (2^-22) and Newton / Halley steps
-// on the fp64 pipe, no slow-path branch.
+// the ends of the exponent range (everything on this path is): one MUFU seed (relative error e <= 2^-22.9) and ONE
+// third-order correction on the fp64 pipe, no slow-path branch.  An fp64 instruction occupies the issue port of its
+// scheduler for two cycles on sm_100a ("issue model"), so these are counted in instructions:
+//   1/a     = r (1 + e + e^2 + O(e^3)),            e = 1 - a r          : 3 instructions, truncation 2^-69
+//   sqrt(a) = a r (1 + e/2 + 3 e^2/8 + O(e^3)),    e = 1 - a r^2        : 5 instructions, truncation 2^-70
+// (two Newton steps plus a residual correction, as in libdevice, cost 4 and 10).  Results are good to about 1 ulp.
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double rcp_fast(double a)
 {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
-    double e = fma(-a, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-a, r, 1.0);
-    return fma(r, e, r);
+    const double e = fma(-a, r, 1.0);
+    return fma(r, fma(e, e, e), r);
 }
 
-// sqrt(a) to 1 ulp; `half_rsqrt` receives 1/(2 sqrt(a)) from the same two Newton steps (a few ulp).
+// sqrt(a); `half_rsqrt` receives 1/(2 sqrt(a)) from the same correction (two more instructions when it is used).
 __device__ __forceinline__ double sqrt_fast(double a, double& half_rsqrt)
 {
     double r;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
-    double g = a * r, h = 0.5 * r;
-    double e = fma(-g, h, 0.5);
-    g = fma(g, e, g);
-    h = fma(h, e, h);
-    e = fma(-g, h, 0.5);
-    g = fma(g, e, g);
-    h = fma(h, e, h);
-    const double d = fma(-g, g, a);
-    half_rsqrt = h;
-    return fma(d, h, g);
+    const double t = a * r;
+    const double e = fma(-t, r, 1.0);
+    const double q = fma(e, 0.375, 0.5) * e;
+    const double hr = 0.5 * r;
+    half_rsqrt = fma(hr, q, hr);
+    return fma(t, q, t);
 }
 __device__ __forceinline__ double sqrt_fast(double a)
 {
