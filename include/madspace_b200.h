@@ -160,6 +160,11 @@ typedef struct ms_gen_config {
     int32_t massive;       /* 1: Newton rescale to `masses` */
     int32_t toy;           /* 1: multiply the weight by the toy integrand */
     int32_t max_iter;      /* Newton cap of the rescale */
+    int32_t tail_unit_jacobian; /* 1: the caller asserts that every grid dimension the phase-space map does not consume
+                              (index >= 3n-4 [+2 with pdf]) has n_bins*(x_{j+1}-x_j) == 1.0 exactly in every bin (e.g. a
+                              uniform grid with a power-of-two bin count), so its Jacobian factor is exactly 1 and the
+                              kernel skips it; 0: those dimensions are drawn and looked up like the others */
+    int32_t reserved;      /* must be 0 */
     double sqrt_s;         /* partonic (pdf=0) or hadronic (pdf=1) CM energy */
     double tau_min;
     double rel_tol;        /* rescale tolerance */

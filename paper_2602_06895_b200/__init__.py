@@ -41,6 +41,7 @@ class ms_rng(C.Structure):
 class ms_gen_config(C.Structure):
     _fields_ = [("n", C.c_int32), ("mapping", C.c_int32), ("grid_dims", C.c_int32), ("grid_bins", C.c_int32),
                 ("pdf", C.c_int32), ("massive", C.c_int32), ("toy", C.c_int32), ("max_iter", C.c_int32),
+                ("tail_unit_jacobian", C.c_int32), ("reserved", C.c_int32),
                 ("sqrt_s", C.c_double), ("tau_min", C.c_double), ("rel_tol", C.c_double), ("toy_reg", C.c_double),
                 ("masses", C.c_double * MS_MAX_N)]
 
@@ -183,12 +184,13 @@ def ms_unweight(N, d_w, d_wmax, r: ms_rng, n_rows, d_rows_in, cap, d_idx, d_w_ou
 
 
 def gen_config(n, mapping="fastrambo", sqrt_s=0.0, grid_dims=0, grid_bins=0, pdf=False, tau_min=0.0, masses=(),
-               rel_tol=1e-14, max_iter=10, toy=False, toy_reg=100.0) -> ms_gen_config:
+               rel_tol=1e-14, max_iter=10, toy=False, toy_reg=100.0, tail_unit_jacobian=False) -> ms_gen_config:
     cfg = ms_gen_config()
     cfg.n, cfg.mapping = n, {"fastrambo": 0, "rambo": 1}[mapping]
     cfg.grid_dims, cfg.grid_bins = grid_dims, grid_bins
     cfg.pdf, cfg.massive, cfg.toy, cfg.max_iter = int(pdf), int(len(masses) > 0), int(toy), max_iter
     cfg.sqrt_s, cfg.tau_min, cfg.rel_tol, cfg.toy_reg = sqrt_s, tau_min, rel_tol, toy_reg
+    cfg.tail_unit_jacobian, cfg.reserved = int(tail_unit_jacobian), 0
     for i, m in enumerate(masses):
         cfg.masses[i] = float(m)
     return cfg

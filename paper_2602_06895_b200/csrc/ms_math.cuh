@@ -346,7 +346,7 @@ __device__ __forceinline__ float root_f32(float y, float inv_k)
 // coefficients serves both sides.  The paper names no method.  Here, branch-free and vote-free:
 //   1. start value in fp32: the FastRambo value (RQF approximates Eq. 62 to a few per cent), or the
 //      leading term sqrt(2(1-r)/(k(k+1))) when 1-r < 1e-3;
-//   2. four Newton steps in fp32 (-> ~1e-7 relative for every k <= 7, measured against 40-digit roots);
+//   2. three (k <= 3) or four Newton steps in fp32 (-> ~1e-7 relative, measured against 40-digit roots);
 //   3. ONE Halley step in fp64 (cubic: 1e-7 -> < 3e-16).
 // Returns false (event weight 0, fail counter) if the Halley step moved w by more than 1e-4 relative, i.e. if stage 2
 // had not converged.
@@ -393,9 +393,9 @@ __device__ __forceinline__ bool rambo_mass_step(double r, double& u, double& omu
             const float y = (2.0f * xf) * rcp_f32((a + 1.0f) + sq);
             w = root_f32(y, 1.0f / K);
         }
-        // ---- 2. four fp32 Newton steps
+        // ---- 2. fp32 Newton steps: three reach ~1.5e-7 for k <= 3, four for k <= 7 (40-digit reference roots)
 #pragma unroll
-        for (int it = 0; it < 4; ++it) {
+        for (int it = 0; it < (K <= 3 ? 3 : 4); ++it) {
             float G = cf[K + 1], H = (K + 1) * cf[K + 1];
 #pragma unroll
             for (int j = K; j >= 2; --j) {

@@ -59,10 +59,12 @@ class HotPath:
         self.fail = torch.zeros(1, dtype=torch.int32, device=self.device)
         self.d_edges = None
         self.grid_dims = self.grid_bins = 0
+        self.tail_unit_jacobian = False
         if spec.edges is not None:
             self.set_grid(spec.edges)
         self.cfg = gen_config(spec.n, spec.mapping, spec.sqrt_s, self.grid_dims, self.grid_bins, spec.pdf, spec.tau_min,
-                              tuple(spec.masses), spec.rel_tol, spec.max_iter, spec.toy, spec.toy_reg)
+                              tuple(spec.masses), spec.rel_tol, spec.max_iter, spec.toy, spec.toy_reg,
+                              tail_unit_jacobian=self.tail_unit_jacobian)
         if spec.unweight:
             self.cap = int(cap) if cap is not None else max(1024, self.N // 64)
             self.wmax = torch.zeros(1, **f64)
@@ -84,6 +86,11 @@ class HotPath:
         if ms_check_grid(h_edges) != 0:
             raise MadSpaceError("ms_check_grid", MS_EGRID)
         self.grid_dims, self.grid_bins = h_edges.shape[0], h_edges.shape[1] - 1
+        # unused trailing dimensions whose bins all have n_bins * width == 1.0 exactly contribute a Jacobian of exactly 1
+        tail = h_edges[self.spec.d_used:]
+        self.tail_unit_jacobian = bool(tail.shape[0] > 0 and np.all(self.grid_bins * np.diff(tail, axis=1) == 1.0))
+        if hasattr(self, "cfg"):
+            self.cfg.tail_unit_jacobian = int(self.tail_unit_jacobian)
         t = torch.from_numpy(h_edges)
         if self.d_edges is None:
             self.d_edges = torch.empty(h_edges.shape, dtype=torch.float64, device=self.device)

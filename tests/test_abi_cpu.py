@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(ms):
 
 def test_struct_layouts_match_the_header(ms):
     assert C.sizeof(ms.ms_rng) == 24
-    assert C.sizeof(ms.ms_gen_config) == 8 * 4 + 4 * 8 + 9 * 8
+    assert C.sizeof(ms.ms_gen_config) == 10 * 4 + 4 * 8 + 9 * 8
 
 
 def test_check_grid(ms):
