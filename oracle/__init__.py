@@ -183,6 +183,20 @@ def massive_rescale(n, sqrt_s, masses, p, w, rel_tol=1e-14, max_iter=10):
     return p2, w2, int(nf)
 
 
+def rambo_massive_reweight(n, x, sqrt_s, masses, exact=False):
+    """Massive phase space by reweighting (strategy (ii), Eq. 68-69).  Returns (p, w, n_bad)."""
+    N = x.shape[1]
+    _chk(x, 3 * n - 4)
+    m = np.ascontiguousarray(masses, dtype=np.float64)
+    assert m.shape[0] == n
+    p = np.empty((4 * (n + 2), N))
+    w = np.empty(N)
+    lib().orc_rambo_massive_reweight.restype = C.c_int64
+    nb = lib().orc_rambo_massive_reweight(C.c_int(int(exact)), C.c_int64(N), C.c_int(n), C.c_double(sqrt_s), _p(m),
+                                          _p(x), _p(p), _p(w), C.c_int64(N))
+    return p, w, int(nb)
+
+
 def pdf_x_sample(s_had, tau_min, r):
     N = r.shape[1]
     _chk(r)

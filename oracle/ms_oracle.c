@@ -396,6 +396,104 @@ void orc_rambo_massless(int64_t N, int n, double sqrt_s, const double *sqrt_s_ar
 }
 
 /* ------------------------------------------------------------------------ */
+/* K-4: massive extension, strategy (ii) of PAPER.md:510-522 -- the one the  */
+/* paper adopts: "mass effects are incorporated through a reweighting of     */
+/* massless phase-space points" (Eq. 68-69).  Step by step:                  */
+/*   K_1 = M_1 - sum_j m_j; K_i = u_2..u_i K_1 with the u_i of the MASSLESS  */
+/*   FastRambo (or exact Rambo) map; M_i = K_i + sum_{j>=i} m_j (Eq. 69, with */
+/*   the sum read as j = i..n: as printed, j = 1..n, K_i would go negative    */
+/*   and contradict the line's own K_n = 0 -- DESIGN.md reading K-4a);       */
+/*   n-1 two-body decays {Q_{i-1}, M_{i-1}} -> {p_{i-1}, m_{i-1}} + {Q_i, M_i}  */
+/*   (Eq. 53-55; two-body momentum Eq. 24);                                   */
+/*   weight = Phi_n(K_1) w_n  prod_{i=2}^{n} rho(M_{i-1},M_i,m_{i-1}) /       */
+/*            rho(K_{i-1},K_i,0)  prod_{i=2}^{n-1} M_i/K_i  (Eq. 68, with the  */
+/*   printed prefactor 1/8 dropped: under the paper's own rho, Eq. 55, the   */
+/*   i = n term rho(K_{n-1},0,0) = 1/8 already sits in the denominator and    */
+/*   the printed form gives 1/8 of the exact volume for n = 2 -- reading K-4b;*/
+/*   pinned by the closed-form two-body volume and the nested-quadrature      */
+/*   massive 4-body volume in tests/test_oracle_massive_rw.py).               */
+/* Returns the number of events with sum m >= sqrt_s (weight 0).              */
+/* ------------------------------------------------------------------------ */
+/* sqrt(lambda(M^2, m1^2, m2^2)) through the textbook factorisation
+ *   lambda = (M - m1 - m2)(M + m1 + m2)(M - m1 + m2)(M + m1 - m2),
+ * with the first factor d = M - m1 - m2 supplied by the caller, who knows it without cancellation:
+ * here M_{i-1} - m_{i-1} - M_i = K_{i-1} - K_i (Eq. 69).  The expanded form a^2+b^2+c^2-2ab-2ac-2bc loses
+ * eps M^4/lambda and would make soft emissions (u_i -> 1) the accuracy limit of the whole oracle. */
+static double sqrt_kallen(double M, double m1, double m2, double d)
+{
+    double lam = d * (M + m1 + m2) * (M - m1 + m2) * (M + m1 - m2);
+    return sqrt(lam > 0.0 ? lam : 0.0);
+}
+
+int64_t orc_rambo_massive_reweight(int exact, int64_t N, int n, double sqrt_s, const double *masses,
+                                   const double *x, double *p, double *w, int64_t ld)
+{
+    double phi1 = orc_phi_n(n, 1.0);
+    double msum[ORC_MAX_N + 2];                            /* msum[i] = sum_{j>=i} m_j, i = 1..n */
+    msum[n + 1] = 0.0;
+    for (int i = n; i >= 1; --i) msum[i] = msum[i + 1] + masses[i - 1];
+    int64_t nbad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nbad)
+    for (int64_t e = 0; e < N; ++e) {
+        double K[ORC_MAX_N + 2], M[ORC_MAX_N + 2], u[ORC_MAX_N + 2], omu2[ORC_MAX_N + 2];
+        double pout[ORC_MAX_N][4];
+        double wn = 1.0, wm = 1.0;
+        K[1] = sqrt_s - msum[1];
+        if (!(K[1] > 0.0)) { w[e] = 0.0; nbad += 1; continue; }
+        M[1] = sqrt_s;
+        for (int i = 2; i <= n - 1; ++i) {
+            int k = n - i;
+            double xi = x[(int64_t)(i - 2) * ld + e];
+            double wf = 1.0;
+            if (exact) orc_rambo_mass_step(xi, k, &u[i], &omu2[i]);
+            else u[i] = fastrambo_mass_step(xi, k, &omu2[i], &wf);
+            wn *= wf;
+            K[i] = u[i] * K[i - 1];
+            M[i] = K[i] + msum[i];                         /* Eq. 69 (reading K-4a) */
+            wm *= M[i] / K[i];                             /* second product of Eq. 68 */
+        }
+        K[n] = 0.0;
+        M[n] = masses[n - 1];
+        /* decay chain, Eq. 53-55 with masses; first product of Eq. 68 alongside */
+        double Q[4] = { M[1], 0.0, 0.0, 0.0 };
+        for (int i = 2; i <= n; ++i) {
+            double Mp = M[i - 1], m1 = masses[i - 2], m2 = M[i];
+            /* K_{i-1} - K_i = K_{i-1} (1 - u_i) = K_{i-1} (1 - u_i^2)/(1 + u_i);  K_n = 0 */
+            double d = (i < n) ? K[i - 1] * omu2[i] / (1.0 + u[i]) : K[i - 1];
+            double sl = sqrt_kallen(Mp, m1, m2, d);
+            double q = sl / (2.0 * Mp);                    /* Eq. 24 */
+            double rho_M = sl / (8.0 * Mp * Mp);           /* Eq. 55 */
+            double rho_K = (i < n) ? omu2[i] / 8.0 : 1.0 / 8.0;   /* Eq. 55 at m = 0: (K_{i-1}^2 - K_i^2)/(8 K_{i-1}^2) */
+            wm *= rho_M / rho_K;
+            double e1 = (Mp * Mp + m1 * m1 - m2 * m2) / (2.0 * Mp);
+            double xc = x[(int64_t)(n - 2 + 2 * (i - 2)) * ld + e], xp = x[(int64_t)(n - 1 + 2 * (i - 2)) * ld + e];
+            double cth = 2.0 * xc - 1.0, sth = 2.0 * sqrt(xc * (1.0 - xc)), phi = 2.0 * M_PI * xp;   /* Eq. 25 */
+            double pr[4] = { e1, q * sth * cos(phi), q * sth * sin(phi), q * cth };
+            double Qr[4] = { Mp - e1, -pr[1], -pr[2], -pr[3] };
+            if (i == 2) {
+                memcpy(pout[0], pr, sizeof pr);
+                memcpy(Q, Qr, sizeof Qr);
+            } else {
+                double Qn[4];
+                boost_to(Q, Mp, pr, pout[i - 2]);
+                boost_to(Q, Mp, Qr, Qn);
+                memcpy(Q, Qn, sizeof Qn);
+            }
+        }
+        memcpy(pout[n - 1], Q, sizeof Q);
+        double in_a[4] = { 0.5 * sqrt_s, 0.0, 0.0, 0.5 * sqrt_s }, in_b[4] = { 0.5 * sqrt_s, 0.0, 0.0, -0.5 * sqrt_s };
+        for (int mu = 0; mu < 4; ++mu) {
+            p[(int64_t)(0 + mu) * ld + e] = in_a[mu];
+            p[(int64_t)(4 + mu) * ld + e] = in_b[mu];
+        }
+        for (int j = 0; j < n; ++j)
+            for (int mu = 0; mu < 4; ++mu) p[(int64_t)(4 * (j + 2) + mu) * ld + e] = pout[j][mu];
+        w[e] = phi1 * pow(K[1], 2 * n - 4) * wn * wm;
+    }
+    return nbad;
+}
+
+/* ------------------------------------------------------------------------ */
 /* F: FastRambo inverse.  Eq. 64 for the masses; angles by */
 /* undoing Eq. 25 in the rest frame of Q_{i-1} (reading F-1..F-5).           */
 /* p: outgoing momenta are rows 8.. ; frame: any frame (Q_1 = sum of p).     */
