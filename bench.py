@@ -82,7 +82,10 @@ def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
         c += ALG_FP64["toy_pair"] * (n - 1)
     if wl.pdf:
         c += ALG_FP64["pdf"] + ALG_FP64["boost_particle"] * n
-    if wl.masses:
+    if wl.masses and wl.massive_mode == "reweight":
+        # per decay: 1-u via rcp (2 + RCP), factorised Kallen (7) + sqrt, 1/(2M) (RCP + 1), q, e_rest (4), weight (5), M_i (1)
+        c += (n - 1) * (2 + RCP + 7 + SQRT + RCP + 1 + 1 + 4 + 5 + 1) + 2
+    elif wl.masses:
         nm = sum(1 for m in wl.masses if m > 0)
         c += ALG_FP64["rescale_start"] + ALG_FP64["rescale_weight"]
         c += RESCALE_EVALUATIONS * (ALG_FP64["rescale_eval_massive"] * nm + ALG_FP64["rescale_eval_massless"] * (n - nm)
@@ -223,7 +226,8 @@ def workload_config(wl, n_gpus):
 def spec_from_workload(wl):
     from paper_2602_06895_b200.pipeline import PathSpec
     return PathSpec(n=wl.n, sqrt_s=wl.sqrt_s, mapping=wl.mapping, edges=wl.grid(), pdf=wl.pdf, tau_min=wl.tau_min,
-                    masses=tuple(wl.masses), toy=wl.toy, toy_reg=ms_inputs.TOY_REG, unweight=wl.unweight,
+                    masses=tuple(wl.masses), massive_mode=wl.massive_mode, toy=wl.toy, toy_reg=ms_inputs.TOY_REG,
+                    unweight=wl.unweight,
                     inverse=wl.inverse, prerun=ms_inputs.PRERUN, seed_events=ms_inputs.SEED_EVENTS,
                     seed_unweight=ms_inputs.SEED_UNWEIGHT)
 

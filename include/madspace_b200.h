@@ -111,6 +111,15 @@ int ms_fastrambo_inverse(int64_t N, int n, const double* d_p, double* d_x, doubl
 int ms_massive_rescale(int64_t N, int n, double sqrt_s, const double* h_masses, double rel_tol, int max_iter,
                        double* d_p, double* d_w, int64_t ld, uint32_t* d_fail, void* stream);
 
+/* ms_rambo_massive_reweight -- massive extension, strategy (ii) of PAPER.md:510-522 (the one MadSpace adopts): the
+ * massless mass chain runs at K_1 = sqrt_s - sum m_j, M_i = K_i + sum_{j>=i} m_j (Eq. 69, reading K-4a), the
+ * n-1 two-body decays use the massive two-body momentum (Eq. 24) and the weight is
+ *   Phi_n(K_1) w_n prod_{i=2..n} rho(M_{i-1},M_i,m_{i-1})/rho(K_{i-1},K_i,0) prod_{i=2..n-1} M_i/K_i   (Eq. 68, reading K-4b).
+ * mapping 0: FastRambo u_i, 1: exact Rambo u_i.  d_x: [3n-4][ld] uniforms or NULL -> Philox.  h_masses: n doubles on
+ * the HOST, sum < sqrt_s (else MS_EKIN).  d_p: [4(n+2)][ld] out, CM frame; d_w: [N] out. */
+int ms_rambo_massive_reweight(int64_t N, int n, int mapping, double sqrt_s, const double* h_masses, const double* d_x,
+                              ms_rng rng, double* d_p, double* d_w, int64_t ld, uint32_t* d_fail, void* stream);
+
 /* ms_pdf_x_boost -- Bjorken-x sampling and lab boost (Eq. 19 with m^2=0, Eq. 21-23;
  * ops r_to_x1x2 and boost_beam; readings X-1, X-2).
  *   phase 0 (sample): tau = tau_min^(1-r_0), x1 = tau^r_1, x2 = tau^(1-r_1);
@@ -157,7 +166,7 @@ typedef struct ms_gen_config {
     int32_t grid_dims;     /* 0: no grid (uniforms used directly); else >= uniforms consumed */
     int32_t grid_bins;
     int32_t pdf;           /* 1: dims 0,1 -> (tau, y); phase space at sqrt(tau s_had); boost to lab */
-    int32_t massive;       /* 1: Newton rescale to `masses` */
+    int32_t massive;       /* 0: massless; 1: Newton rescale to `masses` (strategy i); 2: reweighting (strategy ii, Eq. 68-69) */
     int32_t toy;           /* 1: multiply the weight by the toy integrand */
     int32_t max_iter;      /* Newton cap of the rescale */
     int32_t tail_unit_jacobian; /* 1: the caller asserts that every grid dimension the phase-space map does not consume

@@ -58,6 +58,7 @@ class Workload:
     pdf: bool = False
     tau_min: float = 0.0
     masses: tuple = ()
+    massive_mode: str = "rescale"   # "rescale": strategy (i), Newton; "reweight": strategy (ii), Eq. 68-69
     toy: bool = False
     unweight: bool = False
     inverse: bool = False
@@ -101,6 +102,10 @@ WORKLOADS = {
     "cfg4": Workload("cfg4", n=4, N=1 << 25, sqrt_s=2000.0, grid_dims=0, grid_bins=0, grid_kind="none",
                      mapping="fastrambo", masses=(173.0, 173.0, 0.0, 0.0),
                      note="massive 2->4 (173,173,0,0): FastRambo + Newton rescale"),
+    # not a BASELINE.json config: cfg4's process with the paper's own massive strategy
+    "cfg4rw": Workload("cfg4rw", n=4, N=1 << 25, sqrt_s=2000.0, grid_dims=0, grid_bins=0, grid_kind="none",
+                       mapping="fastrambo", masses=(173.0, 173.0, 0.0, 0.0), massive_mode="reweight",
+                       note="massive 2->4 (173,173,0,0): FastRambo with mass reweighting (Eq. 68-69)"),
     "cfg5": Workload("cfg5", n=8, N=1 << 24, sqrt_s=3000.0, grid_dims=20, grid_bins=128, grid_kind="seeded",
                      mapping="fastrambo", toy=True, unweight=True, inverse=True,
                      note="massless 2->8 FastRambo, seeded 128x20 grid, toy integrand, unweighting, round trip"),

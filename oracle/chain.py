@@ -40,10 +40,14 @@ def oracle_chain(orc, wl: ms_inputs.Workload, events, edges=None):
         energy = wl.sqrt_s
         jx = 1.0
     xs = np.ascontiguousarray(x[off:off + 3 * n - 4])
-    fn = orc.fastrambo if wl.mapping == "fastrambo" else orc.rambo_massless
-    p, w = fn(n, xs, energy)
+    if wl.masses and wl.massive_mode == "reweight":
+        p, w, nbad = orc.rambo_massive_reweight(n, xs, wl.sqrt_s, wl.masses, exact=(wl.mapping == "rambo"))
+        out["nfail"] = nbad
+    else:
+        fn = orc.fastrambo if wl.mapping == "fastrambo" else orc.rambo_massless
+        p, w = fn(n, xs, energy)
     out["p_massless"], out["w_ps"] = p, w
-    if wl.masses:
+    if wl.masses and wl.massive_mode == "rescale":
         p, w, nfail = orc.massive_rescale(n, wl.sqrt_s, wl.masses, p, w)
         out["nfail"] = nfail
     if wl.pdf:

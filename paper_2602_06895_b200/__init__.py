@@ -23,7 +23,7 @@ MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA = 0, -1, -2, -3, -4
 _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA"}
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_rambo_massless", "ms_fastrambo",
-           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
+           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
            "ms_unweight_scratch_bytes", "ms_unweight", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
 
@@ -69,6 +69,7 @@ def lib() -> C.CDLL:
         for name in ("ms_rambo_massless", "ms_fastrambo"):
             getattr(L, name).argtypes = [_i64, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
         L.ms_fastrambo_inverse.argtypes = [_i64, _int, _vp, _vp, _vp, _i64, _vp]
+        L.ms_rambo_massive_reweight.argtypes = [_i64, _int, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
         L.ms_massive_rescale.argtypes = [_i64, _int, _dbl, _vp, _dbl, _int, _vp, _vp, _i64, _vp, _vp]
         L.ms_pdf_x_boost.argtypes = [_i64, _int, _dbl, _dbl, _int, _vp, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp]
         L.ms_toy_integrand.argtypes = [_i64, _int, _dbl, _vp, _vp, _int, _i64, _vp]
@@ -184,11 +185,13 @@ def ms_unweight(N, d_w, d_wmax, r: ms_rng, n_rows, d_rows_in, cap, d_idx, d_w_ou
 
 
 def gen_config(n, mapping="fastrambo", sqrt_s=0.0, grid_dims=0, grid_bins=0, pdf=False, tau_min=0.0, masses=(),
-               rel_tol=1e-14, max_iter=10, toy=False, toy_reg=100.0, tail_unit_jacobian=False) -> ms_gen_config:
+               rel_tol=1e-14, max_iter=10, toy=False, toy_reg=100.0, tail_unit_jacobian=False,
+               massive_mode="rescale") -> ms_gen_config:
     cfg = ms_gen_config()
     cfg.n, cfg.mapping = n, {"fastrambo": 0, "rambo": 1}[mapping]
     cfg.grid_dims, cfg.grid_bins = grid_dims, grid_bins
-    cfg.pdf, cfg.massive, cfg.toy, cfg.max_iter = int(pdf), int(len(masses) > 0), int(toy), max_iter
+    cfg.pdf, cfg.toy, cfg.max_iter = int(pdf), int(toy), max_iter
+    cfg.massive = {"rescale": 1, "reweight": 2}[massive_mode] if len(masses) > 0 else 0
     cfg.sqrt_s, cfg.tau_min, cfg.rel_tol, cfg.toy_reg = sqrt_s, tau_min, rel_tol, toy_reg
     cfg.tail_unit_jacobian, cfg.reserved = int(tail_unit_jacobian), 0
     for i, m in enumerate(masses):
@@ -211,3 +214,13 @@ def ms_probe_write(N, rows, d_out, ld, stream=None) -> None:
 
 def ms_probe_dfma3(blocks, iters, d_sink, stream=None) -> None:
     _check("ms_probe_dfma3", lib().ms_probe_dfma3(blocks, iters, _ptr(d_sink), _stream(stream)))
+
+
+def ms_rambo_massive_reweight(N, n, mapping, sqrt_s, masses: Sequence[float], d_x, r: ms_rng, d_p, d_w, ld,
+                              d_fail=None, stream=None) -> None:
+    if len(masses) != n:
+        raise MadSpaceError("ms_rambo_massive_reweight", MS_EINVAL)
+    h = (C.c_double * len(masses))(*[float(m) for m in masses])
+    _check("ms_rambo_massive_reweight",
+           lib().ms_rambo_massive_reweight(N, n, {"fastrambo": 0, "rambo": 1}[mapping], sqrt_s, C.addressof(h), _ptr(d_x),
+                                           r, _ptr(d_p), _ptr(d_w), ld, _ptr(d_fail), _stream(stream)))

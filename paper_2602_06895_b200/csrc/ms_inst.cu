@@ -30,10 +30,10 @@ static int grid_for(K kernel, int64_t N, size_t smem)
 #if MS_PART == 0 || MS_PART == 1
 constexpr bool kExact = MS_PART == 1;
 
-template <bool MASSIVE, bool PDF, bool TOY, bool ROWS, bool GRID>
+template <int MASSMODE, bool PDF, bool TOY, bool ROWS, bool GRID>
 static cudaError_t launch_gen_t(const GenParams& P, cudaStream_t stream)
 {
-    auto kernel = gen_kernel<MS_N, kExact, MASSIVE, PDF, TOY, ROWS, GRID>;
+    auto kernel = gen_kernel<MS_N, kExact, MASSMODE, PDF, TOY, ROWS, GRID>;
     const size_t smem = GRID ? (size_t)P.grid_dims * P.grid_bins * sizeof(double2) : 0;
     if (smem > 48 * 1024) {
         cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -48,15 +48,19 @@ cudaError_t MS_CAT(launch_gen_fast_, MS_N)
 #else
 cudaError_t MS_CAT(launch_gen_exact_, MS_N)
 #endif
-    (const GenParams& P, bool massive, bool pdf, bool toy, cudaStream_t stream)
+    (const GenParams& P, int massmode, bool pdf, bool toy, cudaStream_t stream)
 {
-    if (P.x_rows != nullptr) return launch_gen_t<false, false, false, true, false>(P, stream);
-    const int sel = (P.grid_dims > 0 ? 8 : 0) | (massive ? 4 : 0) | (pdf ? 2 : 0) | (toy ? 1 : 0);
-#define MS_CASE(v) \
-    case v: return launch_gen_t<((v) & 4) != 0, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 8) != 0>(P, stream);
+    if (P.x_rows != nullptr)
+        return massmode == 2 ? launch_gen_t<2, false, false, true, false>(P, stream)
+                             : launch_gen_t<0, false, false, true, false>(P, stream);
+    const int sel = (P.grid_dims > 0 ? 4 : 0) | (pdf ? 2 : 0) | (toy ? 1 : 0);
+#define MS_CASE(v)                                                                                                  \
+    case v:                                                                                                         \
+        return massmode == 0   ? launch_gen_t<0, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 4) != 0>(P, stream) \
+               : massmode == 1 ? launch_gen_t<1, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 4) != 0>(P, stream) \
+                               : launch_gen_t<2, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 4) != 0>(P, stream);
     switch (sel) {
         MS_CASE(0) MS_CASE(1) MS_CASE(2) MS_CASE(3) MS_CASE(4) MS_CASE(5) MS_CASE(6) MS_CASE(7)
-        MS_CASE(8) MS_CASE(9) MS_CASE(10) MS_CASE(11) MS_CASE(12) MS_CASE(13) MS_CASE(14) MS_CASE(15)
         default: return cudaErrorInvalidValue;
     }
 #undef MS_CASE

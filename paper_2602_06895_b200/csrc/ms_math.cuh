@@ -435,10 +435,11 @@ struct Vec4 {
 };
 
 // One two-body decay {Q_{i-1}, M} -> p_{i-1} + Q_i (Eq. 54-55; angles Eq. 25):
-// massless p of momentum q in the rest frame of Q, boosted by the pure boost taking (M,0) to Q (reading D-3);
-// the recoil is Q - p.  `first`: Q = (M,0,0,0), no boost needed.
+// p has energy e_rest and momentum q in the rest frame of Q (e_rest = q for a massless particle), and is boosted by the
+// pure boost taking (M,0) to Q (reading D-3); the recoil is Q - p.  `first`: Q = (M,0,0,0), no boost needed.
 template <bool FIRST>
-__device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double q, double x_cos, double x_phi, Vec4& p)
+__device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double e_rest, double q, double x_cos, double x_phi,
+                                               Vec4& p)
 {
     const double cth = fma(2.0, x_cos, -1.0);
     const double sth = 2.0 * sqrt_fast(x_cos * (1.0 - x_cos));   // sqrt(1 - cth^2) without cancellation
@@ -447,13 +448,13 @@ __device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double q, doub
     const double qs = q * sth;
     const double rx = qs * cs, ry = qs * sn, rz = q * cth;
     if constexpr (FIRST) {
-        p.e = q; p.x = rx; p.y = ry; p.z = rz;
-        Q.e = M - q; Q.x = -rx; Q.y = -ry; Q.z = -rz;
+        p.e = e_rest; p.x = rx; p.y = ry; p.z = rz;
+        Q.e = M - e_rest; Q.x = -rx; Q.y = -ry; Q.z = -rz;
     } else {
         const double qm = Q.e + M;
         const double inv = rcp_fast(M * qm);
-        const double ep = fma(Q.x, rx, fma(Q.y, ry, fma(Q.z, rz, Q.e * q))) * (inv * qm);
-        const double f = (q + ep) * (inv * M);
+        const double ep = fma(Q.x, rx, fma(Q.y, ry, fma(Q.z, rz, Q.e * e_rest))) * (inv * qm);
+        const double f = (e_rest + ep) * (inv * M);
         p.e = ep;
         p.x = fma(Q.x, f, rx);
         p.y = fma(Q.y, f, ry);

@@ -31,6 +31,8 @@ struct GenParams {
     double grid_bins_f;        // (double)grid_bins
     double jac_scale;          // grid_bins^grid_dims: the VEGAS Jacobian is jac_scale * prod of bin widths
     double masses[kMaxN];
+    double msuf[kMaxN + 1];    // msuf[i] = sum_{j >= i} masses[j] (0-based), msuf[n] = 0: Eq. 69
+    int massmode, _pad2;       // 0 massless, 1 Newton rescale (strategy i), 2 reweighting (strategy ii)
     double* p;                 // [4(n+2)][ld]
     double* w;                 // [N]
     double* x1x2;              // [2][ld] or nullptr

@@ -27,6 +27,7 @@ class PathSpec:
     pdf: bool = False
     tau_min: float = 0.0
     masses: Sequence[float] = ()
+    massive_mode: str = "rescale"       # "rescale" (strategy i, Newton) | "reweight" (strategy ii, Eq. 68-69)
     toy: bool = False
     toy_reg: float = 100.0
     unweight: bool = False
@@ -64,7 +65,7 @@ class HotPath:
             self.set_grid(spec.edges)
         self.cfg = gen_config(spec.n, spec.mapping, spec.sqrt_s, self.grid_dims, self.grid_bins, spec.pdf, spec.tau_min,
                               tuple(spec.masses), spec.rel_tol, spec.max_iter, spec.toy, spec.toy_reg,
-                              tail_unit_jacobian=self.tail_unit_jacobian)
+                              tail_unit_jacobian=self.tail_unit_jacobian, massive_mode=spec.massive_mode)
         if spec.unweight:
             self.cap = int(cap) if cap is not None else max(1024, self.N // 64)
             self.wmax = torch.zeros(1, **f64)

@@ -16,7 +16,7 @@ from oracle.chain import oracle_chain, oracle_uniforms  # noqa: F401  (re-export
 def path_spec(wl: ms_inputs.Workload, edges=None):
     from paper_2602_06895_b200.pipeline import PathSpec
     return PathSpec(n=wl.n, sqrt_s=wl.sqrt_s, mapping=wl.mapping, edges=wl.grid() if edges is None else edges,
-                    pdf=wl.pdf, tau_min=wl.tau_min, masses=tuple(wl.masses), toy=wl.toy, toy_reg=ms_inputs.TOY_REG,
+                    pdf=wl.pdf, tau_min=wl.tau_min, masses=tuple(wl.masses), massive_mode=wl.massive_mode, toy=wl.toy, toy_reg=ms_inputs.TOY_REG,
                     unweight=wl.unweight, inverse=wl.inverse, prerun=ms_inputs.PRERUN,
                     seed_events=ms_inputs.SEED_EVENTS, seed_unweight=ms_inputs.SEED_UNWEIGHT)
 

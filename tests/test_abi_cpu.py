@@ -73,6 +73,8 @@ def test_host_side_argument_errors(ms):
     # masses
     assert _code(ms, ms.ms_massive_rescale, 8, 4, 300.0, (173.0, 173.0, 0.0, 0.0), 1e-14, 10, FAKE, FAKE, 8, None, 0) == ms.MS_EKIN
     assert _code(ms, ms.ms_massive_rescale, 8, 4, 2000.0, (173.0, -1.0, 0.0, 0.0), 1e-14, 10, FAKE, FAKE, 8, None, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_rambo_massive_reweight, 8, 4, "fastrambo", 300.0, (173.0, 173.0, 0.0, 0.0), None, r0, FAKE, FAKE, 8, None, 0) == ms.MS_EKIN
+    assert _code(ms, ms.ms_rambo_massive_reweight, 8, 4, "rambo", 2000.0, (173.0, 173.0, 0.0, 0.0), None, r0, None, FAKE, 8, None, 0) == ms.MS_EINVAL
     # tau_min
     assert _code(ms, ms.ms_pdf_x_boost, 8, 5, 1e8, 1.5, 0, None, r0, FAKE, FAKE, FAKE, None, 8, 0) == ms.MS_EKIN
     assert _code(ms, ms.ms_pdf_x_boost, 8, 5, 1e8, 0.1, 2, None, r0, FAKE, FAKE, FAKE, None, 8, 0) == ms.MS_EINVAL

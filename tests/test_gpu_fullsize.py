@@ -37,7 +37,7 @@ def sample_indices(N, seed):
     return np.unique(np.concatenate(parts)).astype(np.int64)
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg4rw", "cfg5"])
 def test_full_size_step(ms, orc, name):
     from paper_2602_06895_b200.pipeline import HotPath
     wl = ms_inputs.WORKLOADS[name]
