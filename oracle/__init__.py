@@ -197,6 +197,17 @@ def rambo_massive_reweight(n, x, sqrt_s, masses, exact=False):
     return p, w, int(nb)
 
 
+def rambo_massive_reweight_inverse(n, p, masses):
+    """Inverse of rambo_massive_reweight (FastRambo u_i): returns (x, w)."""
+    N = p.shape[1]
+    _chk(p, 4 * (n + 2))
+    m = np.ascontiguousarray(masses, dtype=np.float64)
+    x = np.empty((3 * n - 4, N))
+    w = np.empty(N)
+    lib().orc_rambo_massive_reweight_inverse(C.c_int64(N), C.c_int(n), _p(m), _p(p), _p(x), _p(w), C.c_int64(N))
+    return x, w
+
+
 def pdf_x_sample(s_had, tau_min, r):
     N = r.shape[1]
     _chk(r)

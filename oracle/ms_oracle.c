@@ -539,6 +539,64 @@ void orc_fastrambo_inverse(int64_t N, int n, const double *p, double *x, double 
 }
 
 /* ------------------------------------------------------------------------ */
+/* Inverse of orc_rambo_massive_reweight with the FastRambo u_i (the paper's   */
+/* invertibility check uses massive gg -> t tbar g g kinematics). */
+/* Undo the steps in reverse: Q_i = sum_{j>=i} p_j, M_i = sqrt(Q_i^2) (i < n),  */
+/* K_i = M_i - sum_{j>=i} m_j (Eq. 69, reading K-4a), u_i = K_i / K_{i-1},     */
+/* r_i = G_RQF(u_i^{2k}; c_k) (Eq. 64); angles from p_{i-1} boosted to the rest */
+/* frame of Q_{i-1} (Eq. 25 inverted).  w (optional): the forward weight,      */
+/* Eq. 68 evaluated from the recovered masses and the rest-frame momenta.      */
+/* ------------------------------------------------------------------------ */
+void orc_rambo_massive_reweight_inverse(int64_t N, int n, const double *masses, const double *p, double *x,
+                                        double *w, int64_t ld)
+{
+    double phi1 = orc_phi_n(n, 1.0);
+    double msum[ORC_MAX_N + 2];
+    msum[n + 1] = 0.0;
+    for (int i = n; i >= 1; --i) msum[i] = msum[i + 1] + masses[i - 1];
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < N; ++e) {
+        double pj[ORC_MAX_N + 1][4], Q[ORC_MAX_N + 2][4], M[ORC_MAX_N + 2], K[ORC_MAX_N + 2];
+        for (int j = 1; j <= n; ++j)
+            for (int mu = 0; mu < 4; ++mu) pj[j][mu] = p[(int64_t)(4 * (j + 1) + mu) * ld + e];
+        for (int mu = 0; mu < 4; ++mu) Q[n][mu] = pj[n][mu];
+        for (int i = n - 1; i >= 1; --i)
+            for (int mu = 0; mu < 4; ++mu) Q[i][mu] = Q[i + 1][mu] + pj[i][mu];
+        for (int i = 1; i <= n - 1; ++i) {
+            double m2 = Q[i][0] * Q[i][0] - Q[i][1] * Q[i][1] - Q[i][2] * Q[i][2] - Q[i][3] * Q[i][3];
+            M[i] = sqrt(m2 > 0.0 ? m2 : 0.0);
+            K[i] = M[i] - msum[i];                         /* Eq. 69 */
+        }
+        M[n] = masses[n - 1];
+        K[n] = 0.0;
+        double wn = 1.0, wm = 1.0;
+        for (int i = 2; i <= n - 1; ++i) {
+            int k = n - i;
+            double c = ORC_CK[k];
+            double u = K[i] / K[i - 1];
+            double y = pow(u, 2 * k);                      /* Eq. 60 */
+            x[(int64_t)(i - 2) * ld + e] = orc_rqf_forward(y, c);
+            wn *= (double)(k + 1) * (1.0 - u * u) / orc_rqf_density(y, c);
+            wm *= M[i] / K[i];
+        }
+        for (int i = 2; i <= n; ++i) {
+            double pr[4];
+            boost_from(Q[i - 1], M[i - 1], pj[i - 1], pr);
+            double q = sqrt(pr[1] * pr[1] + pr[2] * pr[2] + pr[3] * pr[3]);
+            double cth = pr[3] / q;
+            double phi = atan2(pr[2], pr[1]);
+            if (phi < 0.0) phi += 2.0 * M_PI;
+            x[(int64_t)(n - 2 + 2 * (i - 2)) * ld + e] = 0.5 * (cth + 1.0);
+            x[(int64_t)(n - 1 + 2 * (i - 2)) * ld + e] = phi / (2.0 * M_PI);
+            /* Eq. 55: rho(M_{i-1}, M_i, m_{i-1}) = sqrt(lambda)/(8 M^2) = q/(4 M);  rho(K_{i-1}, K_i, 0) = (1 - u_i^2)/8 */
+            double uK = K[i] / K[i - 1];
+            wm *= (q / (4.0 * M[i - 1])) / ((1.0 - uK * uK) / 8.0);
+        }
+        if (w) w[e] = phi1 * pow(K[1], 2 * n - 4) * wn * wm;
+    }
+}
+
+/* ------------------------------------------------------------------------ */
 /* K: massive extension, strategy (i) of PAPER.md:510 -- momentum rescaling  */
 /* of classic RAMBO (ref. [64]); formulas restated in reading   */
 /* K-1..K-3 because the paper prints none.  p rows 8.. are read (massless,   */
