@@ -120,6 +120,13 @@ int ms_massive_rescale(int64_t N, int n, double sqrt_s, const double* h_masses, 
 int ms_rambo_massive_reweight(int64_t N, int n, int mapping, double sqrt_s, const double* h_masses, const double* d_x,
                               ms_rng rng, double* d_p, double* d_w, int64_t ld, uint32_t* d_fail, void* stream);
 
+/* ms_rambo_massive_reweight_inverse -- analytic inverse of ms_rambo_massive_reweight with mapping 0 (PAPER.md:740 checks
+ * the invertibility on massive gg -> t tbar g g kinematics): Q_i = sum_{j>=i} p_j, M_i = sqrt(Q_i^2),
+ * K_i = M_i - sum_{j>=i} m_j (Eq. 69), u_i = K_i/K_{i-1}, r_i = G_RQF(u_i^{2k}; c_k) (Eq. 64), angles in the rest frame of
+ * Q_{i-1}.  Reads the outgoing rows 8.. of d_p, writes d_x [3n-4][ld] and, if d_w != NULL, the forward weight. */
+int ms_rambo_massive_reweight_inverse(int64_t N, int n, const double* h_masses, const double* d_p, double* d_x,
+                                      double* d_w, int64_t ld, void* stream);
+
 /* ms_pdf_x_boost -- Bjorken-x sampling and lab boost (Eq. 19 with m^2=0, Eq. 21-23;
  * ops r_to_x1x2 and boost_beam; readings X-1, X-2).
  *   phase 0 (sample): tau = tau_min^(1-r_0), x1 = tau^r_1, x2 = tau^(1-r_1);

@@ -23,7 +23,7 @@ MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA = 0, -1, -2, -3, -4
 _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA"}
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_rambo_massless", "ms_fastrambo",
-           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
+           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
            "ms_unweight_scratch_bytes", "ms_unweight", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
 
@@ -69,6 +69,7 @@ def lib() -> C.CDLL:
         for name in ("ms_rambo_massless", "ms_fastrambo"):
             getattr(L, name).argtypes = [_i64, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
         L.ms_fastrambo_inverse.argtypes = [_i64, _int, _vp, _vp, _vp, _i64, _vp]
+        L.ms_rambo_massive_reweight_inverse.argtypes = [_i64, _int, _vp, _vp, _vp, _vp, _i64, _vp]
         L.ms_rambo_massive_reweight.argtypes = [_i64, _int, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
         L.ms_massive_rescale.argtypes = [_i64, _int, _dbl, _vp, _dbl, _int, _vp, _vp, _i64, _vp, _vp]
         L.ms_pdf_x_boost.argtypes = [_i64, _int, _dbl, _dbl, _int, _vp, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp]
@@ -224,3 +225,12 @@ def ms_rambo_massive_reweight(N, n, mapping, sqrt_s, masses: Sequence[float], d_
     _check("ms_rambo_massive_reweight",
            lib().ms_rambo_massive_reweight(N, n, {"fastrambo": 0, "rambo": 1}[mapping], sqrt_s, C.addressof(h), _ptr(d_x),
                                            r, _ptr(d_p), _ptr(d_w), ld, _ptr(d_fail), _stream(stream)))
+
+
+def ms_rambo_massive_reweight_inverse(N, n, masses: Sequence[float], d_p, d_x, d_w, ld, stream=None) -> None:
+    if len(masses) != n:
+        raise MadSpaceError("ms_rambo_massive_reweight_inverse", MS_EINVAL)
+    h = (C.c_double * len(masses))(*[float(m) for m in masses])
+    _check("ms_rambo_massive_reweight_inverse",
+           lib().ms_rambo_massive_reweight_inverse(N, n, C.addressof(h), _ptr(d_p), _ptr(d_x), _ptr(d_w), ld,
+                                                   _stream(stream)))

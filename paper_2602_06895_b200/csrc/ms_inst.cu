@@ -66,10 +66,15 @@ cudaError_t MS_CAT(launch_gen_exact_, MS_N)
 #undef MS_CASE
 }
 #else
-cudaError_t MS_CAT(launch_inverse_, MS_N)(const InvParams& P, cudaStream_t stream)
+cudaError_t MS_CAT(launch_inverse_, MS_N)(const InvParams& P, bool massive, cudaStream_t stream)
 {
-    auto kernel = inverse_kernel<MS_N>;
-    kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
+    if (massive) {
+        auto kernel = inverse_kernel<MS_N, true>;
+        kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
+    } else {
+        auto kernel = inverse_kernel<MS_N, false>;
+        kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
+    }
     return cudaGetLastError();
 }
 

@@ -45,6 +45,8 @@ struct InvParams {
     double* x;
     double* w;                 // or nullptr
     double phi_unit;
+    double masses[kMaxN];      // massive inverse only
+    double msuf[kMaxN + 1];    // msuf[i] = sum_{j >= i} masses[j]
 };
 
 struct RescaleParams {
