@@ -197,6 +197,17 @@ def rambo_massive_reweight(n, x, sqrt_s, masses, exact=False):
     return p, w, int(nb)
 
 
+def vegas_accumulate(d, n_bins, w, seed, stream=0, event_offset=0, hist=None):
+    """hist[dim][bin of the event's uniform r_dim] += w^2 (VEGAS adaptation, accumulation pass; reading V-4)."""
+    _chk(w)
+    if hist is None:
+        hist = np.zeros((d, n_bins))
+    assert hist.shape == (d, n_bins) and hist.flags["C_CONTIGUOUS"]
+    lib().orc_vegas_accumulate(C.c_int64(w.shape[0]), C.c_int(d), C.c_int(n_bins), _p(w), C.c_uint64(seed),
+                               C.c_uint32(stream), C.c_uint64(event_offset), _p(hist))
+    return hist
+
+
 def rambo_massive_reweight_inverse(n, p, masses):
     """Inverse of rambo_massive_reweight (FastRambo u_i): returns (x, w)."""
     N = p.shape[1]

@@ -151,6 +151,30 @@ void orc_vegas_inverse(int64_t N, int d, int n_bins, const double *edges, const 
 /* W: massless n-body volume, Eq. 81, including (2pi)^(4-3n)  */
 /* (PAPER.md:134, :413).                                                     */
 /* ------------------------------------------------------------------------ */
+/* V-4: VEGAS adaptation, accumulation pass.  PAPER.md:603 names "the classic  */
+/* VEGAS algorithm" and :746 says the grids "are optimized during an initial   */
+/* adaptation phase and are then frozen"; no equations are printed, so this is */
+/* Lepage's algorithm (refs): every event adds the      */
+/* square of its weight w = f J to the bin its uniform r_dim fell into,        */
+/* hist[dim][floor(r_dim n_bins)] += w^2.  The uniforms are the event's own    */
+/* Philox uniforms (reading R-2), so the pass needs only the weights.          */
+/* Sequential, in event order (a reference for sums taken in any order).       */
+/* ------------------------------------------------------------------------ */
+void orc_vegas_accumulate(int64_t N, int d, int n_bins, const double *w, uint64_t seed, uint32_t stream,
+                          uint64_t event_offset, double *hist)
+{
+    for (int64_t e = 0; e < N; ++e) {
+        double w2 = w[e] * w[e];
+        for (int dim = 0; dim < d; ++dim) {
+            double r = orc_uniform(seed, stream, event_offset + (uint64_t)e, (uint32_t)dim);
+            int j = (int)floor(r * (double)n_bins);
+            if (j > n_bins - 1) j = n_bins - 1;
+            hist[(int64_t)dim * n_bins + j] += w2;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------ */
 double orc_phi_n(int n, double E_cm)
 {
     return pow(E_cm, 2 * n - 4) /
