@@ -79,6 +79,17 @@ int ms_check_grid(int d, int n_bins, const double* h_edges);
 int ms_vegas_map(int64_t N, int d, int n_bins, const double* d_edges, int direction,
                  const double* d_in, ms_rng rng, double* d_out, double* d_jac, int64_t ld, void* stream);
 
+/* ms_vegas_accumulate / ms_vegas_refine -- adaptation of the grid before it is frozen ("classic VEGAS",
+ * :746 "optimized during an initial adaptation phase"; no equations printed: Lepage's algorithm, reading V-4).
+ *   accumulate (device): d_hist[dim*n_bins + floor(r_dim n_bins)] += d_w[e]^2 for dim < d, where r_dim is uniform
+ *       `dim` of event rng.event_offset + e (seed / stream as in the generating call); d_hist [d][n_bins] is ADDED to
+ *       (zero it before the first batch of an iteration).  Summation order is unspecified (fp64 atomics).
+ *   refine (host only, no CUDA call): per dimension smooth (d_{j-1} + 6 d_j + d_{j+1})/8, normalise, damp
+ *       ((1-d)/ln(1/d))^alpha, and re-split h_edges so that every new bin receives an equal share; a dimension with an
+ *       all-zero histogram is copied unchanged.  Returns MS_EGRID if h_edges is not a valid grid. */
+int ms_vegas_accumulate(int64_t N, int d, int n_bins, const double* d_w, ms_rng rng, double* d_hist, void* stream);
+int ms_vegas_refine(int d, int n_bins, const double* h_hist, double alpha, const double* h_edges, double* h_edges_out);
+
 /* ms_rambo_massless -- exact flat massless n-body phase space, RamboOnDiet (PAPER.md:405-474,
  * Eq. 52-63): intermediate masses M_i = u_i M_{i-1} with u_i solving Eq. 62 (Newton, reading
  * M-3), then n-1 two-body decays (Eq. 54-55, angles Eq. 25).  Weight is flat: d_w[e] = Phi_n(sqrt_s)

@@ -22,7 +22,7 @@ MS_MAX_N = 9
 MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA = 0, -1, -2, -3, -4
 _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA"}
 
-EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_rambo_massless", "ms_fastrambo",
+EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
            "ms_unweight_scratch_bytes", "ms_unweight", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
         L.ms_unweight_scratch_bytes.argtypes = [_i64]
         L.ms_check_grid.argtypes = [_int, _int, _vp]
         L.ms_fill_uniforms.argtypes = [_i64, _int, ms_rng, _vp, _i64, _vp]
+        L.ms_vegas_accumulate.argtypes = [_i64, _int, _int, _vp, ms_rng, _vp, _vp]
+        L.ms_vegas_refine.argtypes = [_int, _int, _vp, _dbl, _vp, _vp]
         L.ms_vegas_map.argtypes = [_i64, _int, _int, _vp, _int, _vp, ms_rng, _vp, _vp, _i64, _vp]
         for name in ("ms_rambo_massless", "ms_fastrambo"):
             getattr(L, name).argtypes = [_i64, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
@@ -234,3 +236,21 @@ def ms_rambo_massive_reweight_inverse(N, n, masses: Sequence[float], d_p, d_x, d
     _check("ms_rambo_massive_reweight_inverse",
            lib().ms_rambo_massive_reweight_inverse(N, n, C.addressof(h), _ptr(d_p), _ptr(d_x), _ptr(d_w), ld,
                                                    _stream(stream)))
+
+
+def ms_vegas_accumulate(N, d, n_bins, d_w, r: ms_rng, d_hist, stream=None) -> None:
+    _check("ms_vegas_accumulate", lib().ms_vegas_accumulate(N, d, n_bins, _ptr(d_w), r, _ptr(d_hist), _stream(stream)))
+
+
+def ms_vegas_refine(h_hist, h_edges, alpha=0.5):
+    """Host arrays in, refined host edges out (numpy, C-contiguous float64)."""
+    import numpy as np
+    h_hist = np.ascontiguousarray(h_hist, dtype=np.float64)
+    h_edges = np.ascontiguousarray(h_edges, dtype=np.float64)
+    d, nb = h_hist.shape
+    if h_edges.shape != (d, nb + 1):
+        raise MadSpaceError("ms_vegas_refine", MS_EINVAL)
+    out = np.empty_like(h_edges)
+    _check("ms_vegas_refine", lib().ms_vegas_refine(d, nb, h_hist.ctypes.data, float(alpha), h_edges.ctypes.data,
+                                                    out.ctypes.data))
+    return out

@@ -13,7 +13,7 @@ from typing import Optional, Sequence
 import numpy as np
 import torch
 
-from . import (gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
+from . import (ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
                ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID)
 
 
@@ -101,6 +101,18 @@ class HotPath:
     def generate(self, event_offset: int = 0, stream=None) -> None:
         ms_generate(self.cfg, self.N, rng(self.spec.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
                     self.x1x2, self.ld, self.fail, stream)
+
+    def adapt_grid(self, event_offset: int = 0, alpha: float = 0.5, stream=None) -> np.ndarray:
+        """One VEGAS adaptation step from the weights of the last generate(event_offset): accumulate w^2 per bin on the
+        device, refine on the host (tiny tables), install the new grid.  Returns the new host edges."""
+        if self.d_edges is None:
+            raise RuntimeError("adapt_grid needs a grid")
+        hist = torch.zeros((self.grid_dims, self.grid_bins), dtype=torch.float64, device=self.device)
+        ms_vegas_accumulate(self.N, self.grid_dims, self.grid_bins, self.w, rng(self.spec.seed_events, 0, event_offset),
+                            hist, stream)
+        new_edges = ms_vegas_refine(hist.cpu().numpy(), self.d_edges.cpu().numpy(), alpha)
+        self.set_grid(new_edges)
+        return new_edges
 
     def unweight(self, event_offset: int = 0, stream=None) -> None:
         s = self.spec
