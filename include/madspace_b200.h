@@ -173,6 +173,23 @@ int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, 
                 int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted,
                 void* d_scratch, size_t scratch_bytes, int64_t ld, void* stream);
 
+/* Running-maximum unweighting with an overweight allowance ("We estimate the maximum event weight on the
+ * fly, allowing for a user-defined amount of overweight events relative to the total cross section ... a final
+ * unweighting with respect to the final maximum weight is performed"; no formulas printed: DESIGN.md reading U-2).
+ *   ms_weight_histogram (device): d_counts[k] += number of weights whose IEEE-754 bits 62..48 equal k (MS_HIST_BINS =
+ *       32768 bins, 16 per octave); weights that are not positive finite numbers are not counted.  Exact integers, so
+ *       the statistic does not depend on the order or batching of the events.  d_counts is ADDED to.
+ *   ms_wmax_from_histogram (host only): *h_wmax = the smallest bin edge lo_k with
+ *       sum_{j>=k} count_j (lo_{j+1} - lo_k) <= fraction * sum_j count_j lo_j, which guarantees
+ *       sum_{w > w_max} (w - w_max) <= fraction * sum w;  0 for an empty histogram, +inf if no finite edge qualifies.
+ *   Each batch is then unweighted with ms_unweight against the running maximum; the kept events are finally
+ *   unweighted against the final maximum w_f by ms_unweight applied to max(w, w_old) (ms_elementwise_max) with a
+ *   fresh uniform stream: an event kept with probability min(1, w/w_old) survives with min(1, max(w, w_old)/w_f). */
+#define MS_HIST_BINS 32768
+int ms_weight_histogram(int64_t N, const double* d_w, uint64_t* d_counts, void* stream);
+int ms_wmax_from_histogram(const uint64_t* h_counts, double fraction, double* h_wmax);
+int ms_elementwise_max(int64_t N, const double* d_a, const double* d_b, double* d_out, void* stream);
+
 /* ms_generate -- the fused hot path: Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [massive rescale]
  * -> [lab boost] -> [toy integrand] -> weight, one thread per event, everything in registers, only the
  * momenta and the weight are written.  Computes exactly what the chain

@@ -24,7 +24,7 @@ _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECU
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
 
 class MadSpaceError(RuntimeError):
@@ -65,6 +65,9 @@ def lib() -> C.CDLL:
         L.ms_unweight_scratch_bytes.argtypes = [_i64]
         L.ms_check_grid.argtypes = [_int, _int, _vp]
         L.ms_fill_uniforms.argtypes = [_i64, _int, ms_rng, _vp, _i64, _vp]
+        L.ms_weight_histogram.argtypes = [_i64, _vp, _vp, _vp]
+        L.ms_wmax_from_histogram.argtypes = [_vp, _dbl, _vp]
+        L.ms_elementwise_max.argtypes = [_i64, _vp, _vp, _vp, _vp]
         L.ms_vegas_accumulate.argtypes = [_i64, _int, _int, _vp, ms_rng, _vp, _vp]
         L.ms_vegas_refine.argtypes = [_int, _int, _vp, _dbl, _vp, _vp]
         L.ms_vegas_map.argtypes = [_i64, _int, _int, _vp, _int, _vp, ms_rng, _vp, _vp, _i64, _vp]
@@ -254,3 +257,25 @@ def ms_vegas_refine(h_hist, h_edges, alpha=0.5):
     _check("ms_vegas_refine", lib().ms_vegas_refine(d, nb, h_hist.ctypes.data, float(alpha), h_edges.ctypes.data,
                                                     out.ctypes.data))
     return out
+
+
+MS_HIST_BINS = 1 << 15
+
+
+def ms_weight_histogram(N, d_w, d_counts, stream=None) -> None:
+    _check("ms_weight_histogram", lib().ms_weight_histogram(N, _ptr(d_w), _ptr(d_counts), _stream(stream)))
+
+
+def ms_wmax_from_histogram(h_counts, fraction) -> float:
+    """h_counts: numpy uint64/int64 [MS_HIST_BINS] on the host."""
+    import numpy as np
+    h = np.ascontiguousarray(h_counts).view(np.uint64)
+    if h.shape != (MS_HIST_BINS,):
+        raise MadSpaceError("ms_wmax_from_histogram", MS_EINVAL)
+    out = C.c_double(0.0)
+    _check("ms_wmax_from_histogram", lib().ms_wmax_from_histogram(h.ctypes.data, float(fraction), C.addressof(out)))
+    return float(out.value)
+
+
+def ms_elementwise_max(N, d_a, d_b, d_out, stream=None) -> None:
+    _check("ms_elementwise_max", lib().ms_elementwise_max(N, _ptr(d_a), _ptr(d_b), _ptr(d_out), _stream(stream)))

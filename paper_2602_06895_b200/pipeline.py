@@ -13,7 +13,8 @@ from typing import Optional, Sequence
 import numpy as np
 import torch
 
-from . import (ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
+from . import (ms_elementwise_max, ms_weight_histogram, ms_wmax_from_histogram, MS_HIST_BINS,
+               ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
                ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID)
 
 
@@ -151,3 +152,67 @@ class HotPath:
         if self.spec.inverse:
             k += 2 if self.d_edges is not None else 1
         return k
+
+
+class RunningUnweighter:
+    """Unweighting against a running maximum weight with an overweight allowance (reading U-2),
+    batch by batch on the device: exact weight histogram -> w_max on the host (32768 counts) -> partial unweighting of
+    the batch (ms_unweight) -> kept (global index, weight, w_max at the time); finalize() re-unweights the kept events
+    against the final maximum.  Marshalling and buffer ownership only: every arithmetic step is a library call."""
+
+    def __init__(self, fraction: float, seed: int, device="cuda:0", n_rows: int = 0):
+        self.fraction, self.seed, self.device = float(fraction), int(seed), torch.device(device)
+        self.counts = torch.zeros(MS_HIST_BINS, dtype=torch.int64, device=self.device)
+        self.w_max = 0.0
+        self.trace = []
+        self.kept_idx, self.kept_w, self.kept_old, self.kept_rows = [], [], [], []
+        self.n_rows = n_rows
+
+    def add_batch(self, w: torch.Tensor, N: int, event_offset: int, rows: Optional[torch.Tensor] = None, ld: int = 0,
+                  stream=None) -> int:
+        ms_weight_histogram(N, w, self.counts, stream)
+        self.w_max = max(self.w_max, ms_wmax_from_histogram(self.counts.cpu().numpy(), self.fraction))
+        self.trace.append(self.w_max)
+        f64 = dict(dtype=torch.float64, device=self.device)
+        d_wmax = torch.tensor([self.w_max], **f64)
+        cap = N
+        idx = torch.empty(cap, dtype=torch.int64, device=self.device)
+        w_out = torch.empty(cap, **f64)
+        n_acc = torch.zeros(1, dtype=torch.int64, device=self.device)
+        sb = ms_unweight_scratch_bytes(N)
+        scratch = torch.empty(sb, dtype=torch.uint8, device=self.device)
+        use_rows = rows is not None and self.n_rows > 0
+        rows_out = torch.empty((self.n_rows, cap), **f64) if use_rows else None
+        ms_unweight(N, w, d_wmax, rng(self.seed, 1, event_offset), self.n_rows if use_rows else 0, rows if use_rows else None,
+                    cap, idx, w_out, rows_out, n_acc, scratch, sb, ld if use_rows else N, stream)
+        k = int(n_acc.item())
+        self.kept_idx.append(idx[:k] + event_offset)
+        self.kept_w.append(w[idx[:k]])                       # gather of the kept weights (indexing, no arithmetic)
+        self.kept_old.append(torch.full((k,), self.w_max, **f64))
+        if use_rows:
+            self.kept_rows.append(rows_out[:, :k])
+        return k
+
+    def finalize(self, stream=None):
+        """Returns (global indices, output weights, rows or None) of the finally unweighted events."""
+        f64 = dict(dtype=torch.float64, device=self.device)
+        idx_all = torch.cat(self.kept_idx) if self.kept_idx else torch.empty(0, dtype=torch.int64, device=self.device)
+        K = idx_all.numel()
+        if K == 0:
+            return idx_all, torch.empty(0, **f64), None
+        pad = K + (K & 1)
+        w_all, old_all = torch.zeros(pad, **f64), torch.zeros(pad, **f64)
+        w_all[:K] = torch.cat(self.kept_w)
+        old_all[:K] = torch.cat(self.kept_old)
+        w_eff = torch.empty(pad, **f64)
+        ms_elementwise_max(K, w_all, old_all, w_eff, stream)
+        d_wmax = torch.tensor([self.w_max], **f64)
+        fin = torch.empty(K, dtype=torch.int64, device=self.device)
+        w_out = torch.empty(K, **f64)
+        n_acc = torch.zeros(1, dtype=torch.int64, device=self.device)
+        sb = ms_unweight_scratch_bytes(K)
+        scratch = torch.empty(sb, dtype=torch.uint8, device=self.device)
+        ms_unweight(K, w_eff, d_wmax, rng(self.seed, 2, 0), 0, None, K, fin, w_out, None, n_acc, scratch, sb, pad, stream)
+        k = int(n_acc.item())
+        rows = torch.cat(self.kept_rows, dim=1)[:, fin[:k]] if self.kept_rows else None
+        return idx_all[fin[:k]], w_out[:k], rows

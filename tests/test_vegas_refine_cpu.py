@@ -45,3 +45,23 @@ def test_refine_fixed_points_and_errors(ms):
     assert e.value.code == ms.MS_EINVAL
     with pytest.raises(ms.MadSpaceError):
         ms.ms_vegas_refine(np.ones((d, nb - 1)), edges)
+
+
+def test_wmax_from_histogram_matches_the_oracle(ms):
+    """ms_wmax_from_histogram is host-only code: identical doubles to the oracle's walk over the same counts."""
+    from oracle import running_unweight as ru
+    rs = np.random.Generator(np.random.Philox(key=31))
+    for sigma in (0.5, 2.0, 4.0):
+        w = np.exp(sigma * rs.standard_normal(100000))
+        counts = ru.histogram(w)
+        for f in (0.0, 1e-4, 1e-3, 1e-2, 0.3, 1.0, 5.0):
+            assert ms.ms_wmax_from_histogram(counts, f) == ru.wmax_from_histogram(counts, f)
+    empty = np.zeros(ru.N_BINS, dtype=np.int64)
+    assert ms.ms_wmax_from_histogram(empty, 1e-3) == 0.0
+    top = empty.copy()
+    top[0x7FEF] = 1
+    assert ms.ms_wmax_from_histogram(top, 1e-3) == float("inf") == ru.wmax_from_histogram(top, 1e-3)
+    with pytest.raises(ms.MadSpaceError):
+        ms.ms_wmax_from_histogram(empty, -1.0)
+    with pytest.raises(ms.MadSpaceError):
+        ms.ms_wmax_from_histogram(empty[:100], 1e-3)
