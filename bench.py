@@ -330,25 +330,37 @@ def run_ours(args):
 
     # ---- end to end through the C ABI with HOST buffers: grid table H2D and the unweighted sample D2H every step
     h_edges = torch.from_numpy(wl.grid()).pin_memory() if wl.grid() is not None else None
-    d2h = []
+    d2h_counter = [0]
     if wl.unweight:
-        d2h = [(hp.n_acc, torch.empty(1, dtype=torch.int64).pin_memory()),
-               (hp.idx, torch.empty(hp.cap, dtype=torch.int64).pin_memory()),
-               (hp.w_out, torch.empty(hp.cap, dtype=torch.float64).pin_memory()),
-               (hp.rows_out, torch.empty((hp.spec.rows_p, hp.cap), dtype=torch.float64).pin_memory())]
+        # what a generator hands to the host is the unweighted sample: first the accepted count (8 bytes), then exactly
+        # that many entries of idx, w_out and every momentum row
+        h_nacc = torch.empty(1, dtype=torch.int64).pin_memory()
+        h_idx = torch.empty(hp.cap, dtype=torch.int64).pin_memory()
+        h_wout = torch.empty(hp.cap, dtype=torch.float64).pin_memory()
+        h_rows = torch.empty((hp.spec.rows_p, hp.cap), dtype=torch.float64).pin_memory()
     else:
         d2h = [(hp.w, torch.empty(hp.ld, dtype=torch.float64).pin_memory()),
                (hp.p, torch.empty((hp.spec.rows_p, hp.ld), dtype=torch.float64).pin_memory())]
     h2d_bytes = h_edges.numel() * 8 if h_edges is not None else 0
-    d2h_bytes = sum(h.numel() * h.element_size() for _, h in d2h)
 
     def e2e_step():
         if h_edges is not None:
             hp.d_edges.copy_(h_edges, non_blocking=True)
         hp.step(offset)
-        for d, h in d2h:
-            h.copy_(d, non_blocking=True)
-        torch.cuda.current_stream().synchronize()          # the host consumes the step's result
+        cur = torch.cuda.current_stream()
+        if wl.unweight:
+            h_nacc.copy_(hp.n_acc, non_blocking=True)
+            cur.synchronize()
+            k = min(int(h_nacc[0]), hp.cap)
+            h_idx[:k].copy_(hp.idx[:k], non_blocking=True)
+            h_wout[:k].copy_(hp.w_out[:k], non_blocking=True)
+            h_rows[:, :k].copy_(hp.rows_out[:, :k], non_blocking=True)
+            d2h_counter[0] = 8 + k * 8 * (2 + hp.spec.rows_p)
+        else:
+            for d, h in d2h:
+                h.copy_(d, non_blocking=True)
+            d2h_counter[0] = sum(h.numel() * h.element_size() for _, h in d2h)
+        cur.synchronize()                                  # the host consumes the step's result
 
     e2e_step()
     barrier()
@@ -404,11 +416,11 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic (Philox-seeded uniforms; seeded VEGAS grid stands in for an adapted one)",
             "config": workload_config(wl, world), "clocks": clocks,
-            "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+            "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_counter[0],
                     "wall_value": total_events / t_e2e_wall,
                     "what": "grid table H2D from pinned memory + whole step + D2H of %s, host waits every step"
-                            % ("the accepted count and the compacted unweighted sample (idx, w_out, momentum rows; cap %d)" % hp.cap
-                               if wl.unweight else "all momenta and weights")},
+                            % ("the accepted count, then exactly that many entries of the compacted unweighted sample "
+                               "(idx, w_out, %d momentum rows)" % hp.spec.rows_p if wl.unweight else "all momenta and weights")},
             "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "stage_ms": stage_ms, "cpu_baseline": cb,
             "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
                             "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
