@@ -328,46 +328,85 @@ def run_ours(args):
     counts = gather_counts(n_acc_local)
     offsets = output_offsets(counts)
 
-    # ---- end to end through the C ABI with HOST buffers: grid table H2D and the unweighted sample D2H every step
+    # ---- end to end through the public API with HOST buffers: every step copies its input (the grid table) from pinned
+    # host memory and the host reads the step's result.  For a generator the result is the unweighted sample: the
+    # accepted count and that many entries of idx, w_out and every momentum row.  The read-back is pipelined the way a
+    # production driver would do it ("CPU work overlapped"): two sets of buffers, an upload and a download
+    # stream, and the host consumes step k-1 while the device runs step k.
     h_edges = torch.from_numpy(wl.grid()).pin_memory() if wl.grid() is not None else None
+    h2d_bytes = h_edges.numel() * 8 if h_edges is not None else 0
     d2h_counter = [0]
     if wl.unweight:
-        # what a generator hands to the host is the unweighted sample: first the accepted count (8 bytes), then exactly
-        # that many entries of idx, w_out and every momentum row
-        h_nacc = torch.empty(1, dtype=torch.int64).pin_memory()
-        h_idx = torch.empty(hp.cap, dtype=torch.int64).pin_memory()
-        h_wout = torch.empty(hp.cap, dtype=torch.float64).pin_memory()
-        h_rows = torch.empty((hp.spec.rows_p, hp.cap), dtype=torch.float64).pin_memory()
+        # output capacity of the e2e buffers: next power of two above twice the count seen in the device-resident run
+        cap_e2e = min(hp.cap, max(1024, 1 << (2 * max(n_acc_local, 1) - 1).bit_length()))
+        hps = [HotPath(spec_from_workload(wl), N, dev, cap=cap_e2e) for _ in range(2)]
+        up_stream, down_stream = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+        rows_p = hp.spec.rows_p
+        hb = [dict(nacc=torch.empty(1, dtype=torch.int64).pin_memory(),
+                   idx=torch.empty(cap_e2e, dtype=torch.int64).pin_memory(),
+                   wout=torch.empty(cap_e2e, dtype=torch.float64).pin_memory(),
+                   rows=torch.empty((rows_p, cap_e2e), dtype=torch.float64).pin_memory()) for _ in range(2)]
+        ev_grid = [torch.cuda.Event() for _ in range(2)]
+        ev_done = [torch.cuda.Event() for _ in range(2)]
+        ev_copied = [torch.cuda.Event() for _ in range(2)]
+
+        def launch(k):
+            s, h = k % 2, hps[k % 2]
+            if h_edges is not None:                        # this step's input, uploaded while the previous step runs
+                with torch.cuda.stream(up_stream):
+                    h.d_edges.copy_(h_edges, non_blocking=True)
+                    ev_grid[s].record(up_stream)
+                stream.wait_event(ev_grid[s])
+            h.step(offset)
+            ev_done[s].record(stream)
+            with torch.cuda.stream(down_stream):           # whole contiguous buffers: plain async memcpys into pinned memory
+                down_stream.wait_event(ev_done[s])
+                hb[s]["nacc"].copy_(h.n_acc, non_blocking=True)
+                hb[s]["idx"].copy_(h.idx, non_blocking=True)
+                hb[s]["wout"].copy_(h.w_out, non_blocking=True)
+                hb[s]["rows"].copy_(h.rows_out, non_blocking=True)
+                ev_copied[s].record(down_stream)
+
+        def consume(k):
+            s = k % 2
+            ev_copied[s].synchronize()                     # the host has this step's sample
+            n = int(hb[s]["nacc"][0])
+            if n > cap_e2e:
+                raise SystemExit("bench.py: %d accepted events exceed the e2e capacity %d" % (n, cap_e2e))
+            d2h_counter[0] = 8 + cap_e2e * 8 * (2 + rows_p)
+            return n
+
+        def e2e_run(steps):
+            launch(0)
+            for k in range(1, steps):
+                launch(k)
+                consume(k - 1)
+            consume(steps - 1)
+            stream.wait_event(ev_copied[(steps - 1) % 2])  # the timed region ends when the last sample is on the host
+        e2e_what = ("every step: grid table H2D from pinned memory, the whole step, D2H of the accepted count and of the "
+                    "compacted unweighted sample buffers (idx, w_out, %d momentum rows; capacity %d entries); transfers "
+                    "on their own streams with two buffer sets, the host consumes step k-1 while step k runs"
+                    % (rows_p, cap_e2e))
     else:
         d2h = [(hp.w, torch.empty(hp.ld, dtype=torch.float64).pin_memory()),
                (hp.p, torch.empty((hp.spec.rows_p, hp.ld), dtype=torch.float64).pin_memory())]
-    h2d_bytes = h_edges.numel() * 8 if h_edges is not None else 0
 
-    def e2e_step():
-        if h_edges is not None:
-            hp.d_edges.copy_(h_edges, non_blocking=True)
-        hp.step(offset)
-        cur = torch.cuda.current_stream()
-        if wl.unweight:
-            h_nacc.copy_(hp.n_acc, non_blocking=True)
-            cur.synchronize()
-            k = min(int(h_nacc[0]), hp.cap)
-            h_idx[:k].copy_(hp.idx[:k], non_blocking=True)
-            h_wout[:k].copy_(hp.w_out[:k], non_blocking=True)
-            h_rows[:, :k].copy_(hp.rows_out[:, :k], non_blocking=True)
-            d2h_counter[0] = 8 + k * 8 * (2 + hp.spec.rows_p)
-        else:
-            for d, h in d2h:
-                h.copy_(d, non_blocking=True)
-            d2h_counter[0] = sum(h.numel() * h.element_size() for _, h in d2h)
-        cur.synchronize()                                  # the host consumes the step's result
+        def e2e_run(steps):
+            for _ in range(steps):
+                if h_edges is not None:
+                    hp.d_edges.copy_(h_edges, non_blocking=True)
+                hp.step(offset)
+                for d_t, h_t in d2h:
+                    h_t.copy_(d_t, non_blocking=True)
+                d2h_counter[0] = sum(h_t.numel() * h_t.element_size() for _, h_t in d2h)
+                torch.cuda.current_stream().synchronize()  # the host consumes the step's result
+        e2e_what = "grid table H2D from pinned memory + whole step + D2H of all momenta and weights, host waits every step"
 
-    e2e_step()
+    e2e_run(2)
     barrier()
     t0 = time.perf_counter()
     ev[0].record(stream)
-    for _ in range(args.steps):
-        e2e_step()
+    e2e_run(args.steps)
     ev[1].record(stream)
     barrier()
     t_e2e_wall = time.perf_counter() - t0
@@ -418,9 +457,7 @@ def run_ours(args):
             "config": workload_config(wl, world), "clocks": clocks,
             "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_counter[0],
                     "wall_value": total_events / t_e2e_wall,
-                    "what": "grid table H2D from pinned memory + whole step + D2H of %s, host waits every step"
-                            % ("the accepted count, then exactly that many entries of the compacted unweighted sample "
-                               "(idx, w_out, %d momentum rows)" % hp.spec.rows_p if wl.unweight else "all momenta and weights")},
+                    "what": e2e_what},
             "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "stage_ms": stage_ms, "cpu_baseline": cb,
             "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
                             "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
