@@ -138,6 +138,18 @@ int ms_rambo_massive_reweight(int64_t N, int n, int mapping, double sqrt_s, cons
 int ms_rambo_massive_reweight_inverse(int64_t N, int n, const double* h_masses, const double* d_p, double* d_x,
                                       double* d_w, int64_t ld, void* stream);
 
+/* ms_chili -- the Chili mapping (Eq. 70-77; readings C-1..C-5): particles 1..n-1 in
+ * (pT, y, phi) -- pT by Eq. 72 if h_pt_min[i] > 0, else Eq. 73 with lambda_C = m_i or 1 GeV; |y| <= y_max(m_T) of Eq. 74,
+ * further limited by h_y_cut[i] > 0; phi from the current recoil direction (Eq. 75) --, particle n by transverse recoil
+ * (Eq. 76) and a rapidity in |y| <= y_max(m_T,n), incoming momenta from E+- (Eq. 77).  3n-2 uniforms per event:
+ * (r_pT, r_y, r_phi) per generated particle, then r_y of the last one.
+ *   d_w[e] = density of dPhi_n dx1 dx2 (incl. (2 pi)^(4-3n); no flux, no PDFs), 0 outside the technical cut
+ *            E+- <= sqrt(s_lab) or where Eq. 74 has no solution;  d_x1x2 (optional) = E+-/sqrt(s_lab).
+ *   h_masses, h_pt_min, h_y_cut: n doubles on the HOST each, or NULL (all zero).  d_x: [3n-2][ld] or NULL -> Philox.
+ *   d_p: [4(n+2)][ld] out, lab frame. */
+int ms_chili(int64_t N, int n, double s_lab, const double* h_masses, const double* h_pt_min, const double* h_y_cut,
+             const double* d_x, ms_rng rng, double* d_p, double* d_w, double* d_x1x2, int64_t ld, void* stream);
+
 /* ms_pdf_x_boost -- Bjorken-x sampling and lab boost (Eq. 19 with m^2=0, Eq. 21-23;
  * ops r_to_x1x2 and boost_beam; readings X-1, X-2).
  *   phase 0 (sample): tau = tau_min^(1-r_0), x1 = tau^r_1, x2 = tau^(1-r_1);

@@ -23,7 +23,7 @@ MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA = 0, -1, -2, -3, -4
 _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA"}
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
-           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
+           "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
            "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
 
@@ -74,6 +74,7 @@ def lib() -> C.CDLL:
         for name in ("ms_rambo_massless", "ms_fastrambo"):
             getattr(L, name).argtypes = [_i64, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
         L.ms_fastrambo_inverse.argtypes = [_i64, _int, _vp, _vp, _vp, _i64, _vp]
+        L.ms_chili.argtypes = [_i64, _int, _dbl, _vp, _vp, _vp, _vp, ms_rng, _vp, _vp, _vp, _i64, _vp]
         L.ms_rambo_massive_reweight_inverse.argtypes = [_i64, _int, _vp, _vp, _vp, _vp, _i64, _vp]
         L.ms_rambo_massive_reweight.argtypes = [_i64, _int, _int, _dbl, _vp, _vp, ms_rng, _vp, _vp, _i64, _vp, _vp]
         L.ms_massive_rescale.argtypes = [_i64, _int, _dbl, _vp, _dbl, _int, _vp, _vp, _i64, _vp, _vp]
@@ -279,3 +280,16 @@ def ms_wmax_from_histogram(h_counts, fraction) -> float:
 
 def ms_elementwise_max(N, d_a, d_b, d_out, stream=None) -> None:
     _check("ms_elementwise_max", lib().ms_elementwise_max(N, _ptr(d_a), _ptr(d_b), _ptr(d_out), _stream(stream)))
+
+
+def ms_chili(N, n, s_lab, masses, pt_min, y_cut, d_x, r: ms_rng, d_p, d_w, d_x1x2, ld, stream=None) -> None:
+    def harr(v):
+        if v is None:
+            return None, None
+        if len(v) != n:
+            raise MadSpaceError("ms_chili", MS_EINVAL)
+        a = (C.c_double * n)(*[float(t) for t in v])
+        return a, C.addressof(a)
+    keep = [harr(masses), harr(pt_min), harr(y_cut)]
+    _check("ms_chili", lib().ms_chili(N, n, s_lab, keep[0][1], keep[1][1], keep[2][1], _ptr(d_x), r, _ptr(d_p), _ptr(d_w),
+                                      _ptr(d_x1x2), ld, _stream(stream)))

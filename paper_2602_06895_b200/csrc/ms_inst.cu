@@ -78,6 +78,18 @@ cudaError_t MS_CAT(launch_inverse_, MS_N)(const InvParams& P, bool massive, cuda
     return cudaGetLastError();
 }
 
+cudaError_t MS_CAT(launch_chili_, MS_N)(const ChiliParams& P, cudaStream_t stream)
+{
+    if (P.x_rows != nullptr) {
+        auto kernel = chili_kernel<MS_N, true>;
+        kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
+    } else {
+        auto kernel = chili_kernel<MS_N, false>;
+        kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
+    }
+    return cudaGetLastError();
+}
+
 cudaError_t MS_CAT(launch_rescale_, MS_N)(const RescaleParams& P, cudaStream_t stream)
 {
     auto kernel = rescale_kernel<MS_N>;

@@ -49,6 +49,22 @@ struct InvParams {
     double msuf[kMaxN + 1];    // msuf[i] = sum_{j >= i} masses[j]
 };
 
+struct ChiliParams {
+    int64_t N, ld;
+    PhiloxKey key;
+    const double* x_rows;      // [3n-2][ld] uniforms, or nullptr -> Philox in-kernel
+    double s_lab, sqrt_s;
+    double weight_unit;        // (2 pi)^(4-3n) * 2 / s_lab
+    double inv_ptmax2;         // 1 / pT_max^2, pT_max = sqrt(s_lab)/2 (Eq. 71)
+    double masses[kMaxN];
+    double inv_ptmin2[kMaxN];  // 1 / pT_min^2 (Eq. 72) or 0 -> Eq. 73
+    double lambda_c[kMaxN];    // regulator of Eq. 73: the mass, or 1 for a massless particle
+    double y_cut[kMaxN];       // > 0: |y| <= y_cut; else no rapidity cut
+    double* p;                 // [4(n+2)][ld]
+    double* w;                 // [N]
+    double* x1x2;              // [2][ld] or nullptr
+};
+
 struct RescaleParams {
     int64_t N, ld;
     double sqrt_s, rel_tol;
