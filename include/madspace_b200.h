@@ -185,6 +185,27 @@ int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, 
                 int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted,
                 void* d_scratch, size_t scratch_bytes, int64_t ld, void* stream);
 
+/* Observables, cuts and weighted histograms (Sec. 3.2.4-3.2.5; scales Eq. 79-80; the paper names the
+ * observables without formulas: DESIGN.md reading O-1).  Particle indices a, b count row blocks: 0, 1 incoming,
+ * 2.. outgoing.  phi in (-pi, pi], theta in [0, pi], dphi folded into [0, pi], deta = |eta_a - eta_b|,
+ * dR = sqrt(deta^2 + dphi^2), mass = sqrt(max((p_a + p_b)^2, 0)); event level: sqrt(s-hat) from the incoming rows,
+ * E_T^tot = sum E pT/|p| (Eq. 79) and H_T = sum sqrt(m^2 + pT^2) (Eq. 80, m^2 = max(E^2 - |p|^2, 0)) over the first n_out
+ * outgoing particles.
+ *   ms_observable:     d_obs[e] = observable `kind` of event e.
+ *   ms_cut:            d_w[e] = 0 unless lo <= d_obs[e] <= hi (+-infinity allowed; a NaN observable fails the cut).
+ *   ms_histogram_fill: d_sum_w / d_sum_w2 [n_bins + 2] += sum of w / w^2 per slot; slot 0 = underflow, 1..n_bins the
+ *                      uniform bins of [lo, hi), n_bins + 1 = overflow; NaN observables are skipped.  Summation order
+ *                      is unspecified (fp64 atomics). */
+enum {
+    MS_OBS_E = 0, MS_OBS_PX, MS_OBS_PY, MS_OBS_PZ, MS_OBS_PT, MS_OBS_PABS, MS_OBS_PHI, MS_OBS_THETA, MS_OBS_Y, MS_OBS_ABSY,
+    MS_OBS_ETA, MS_OBS_ABSETA, MS_OBS_DPHI, MS_OBS_DETA, MS_OBS_DR, MS_OBS_MASS, MS_OBS_SQRT_SHAT, MS_OBS_ET_TOT, MS_OBS_HT,
+    MS_OBS_COUNT
+};
+int ms_observable(int64_t N, int kind, int a, int b, int n_out, const double* d_p, double* d_obs, int64_t ld, void* stream);
+int ms_cut(int64_t N, const double* d_obs, double lo, double hi, double* d_w, void* stream);
+int ms_histogram_fill(int64_t N, const double* d_obs, const double* d_w, double lo, double hi, int n_bins, double* d_sum_w,
+                      double* d_sum_w2, void* stream);
+
 /* Running-maximum unweighting with an overweight allowance ("We estimate the maximum event weight on the
  * fly, allowing for a user-defined amount of overweight events relative to the total cross section ... a final
  * unweighting with respect to the final maximum weight is performed"; no formulas printed: DESIGN.md reading U-2).

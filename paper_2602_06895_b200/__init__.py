@@ -24,7 +24,7 @@ _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECU
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
 
 class MadSpaceError(RuntimeError):
@@ -65,6 +65,9 @@ def lib() -> C.CDLL:
         L.ms_unweight_scratch_bytes.argtypes = [_i64]
         L.ms_check_grid.argtypes = [_int, _int, _vp]
         L.ms_fill_uniforms.argtypes = [_i64, _int, ms_rng, _vp, _i64, _vp]
+        L.ms_observable.argtypes = [_i64, _int, _int, _int, _int, _vp, _vp, _i64, _vp]
+        L.ms_cut.argtypes = [_i64, _vp, _dbl, _dbl, _vp, _vp]
+        L.ms_histogram_fill.argtypes = [_i64, _vp, _vp, _dbl, _dbl, _int, _vp, _vp, _vp]
         L.ms_weight_histogram.argtypes = [_i64, _vp, _vp, _vp]
         L.ms_wmax_from_histogram.argtypes = [_vp, _dbl, _vp]
         L.ms_elementwise_max.argtypes = [_i64, _vp, _vp, _vp, _vp]
@@ -293,3 +296,21 @@ def ms_chili(N, n, s_lab, masses, pt_min, y_cut, d_x, r: ms_rng, d_p, d_w, d_x1x
     keep = [harr(masses), harr(pt_min), harr(y_cut)]
     _check("ms_chili", lib().ms_chili(N, n, s_lab, keep[0][1], keep[1][1], keep[2][1], _ptr(d_x), r, _ptr(d_p), _ptr(d_w),
                                       _ptr(d_x1x2), ld, _stream(stream)))
+
+
+OBS_KINDS = ("E", "PX", "PY", "PZ", "PT", "PABS", "PHI", "THETA", "Y", "ABSY", "ETA", "ABSETA", "DPHI", "DETA", "DR", "MASS",
+             "SQRT_SHAT", "ET_TOT", "HT")
+
+
+def ms_observable(N, kind: str, a, b, n_out, d_p, d_obs, ld, stream=None) -> None:
+    _check("ms_observable", lib().ms_observable(N, OBS_KINDS.index(kind), a, b, n_out, _ptr(d_p), _ptr(d_obs), ld,
+                                                _stream(stream)))
+
+
+def ms_cut(N, d_obs, lo, hi, d_w, stream=None) -> None:
+    _check("ms_cut", lib().ms_cut(N, _ptr(d_obs), float(lo), float(hi), _ptr(d_w), _stream(stream)))
+
+
+def ms_histogram_fill(N, d_obs, d_w, lo, hi, n_bins, d_sum_w, d_sum_w2, stream=None) -> None:
+    _check("ms_histogram_fill", lib().ms_histogram_fill(N, _ptr(d_obs), _ptr(d_w), float(lo), float(hi), n_bins,
+                                                        _ptr(d_sum_w), _ptr(d_sum_w2), _stream(stream)))
