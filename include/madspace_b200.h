@@ -185,6 +185,15 @@ int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, 
                 int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted,
                 void* d_scratch, size_t scratch_bytes, int64_t ld, void* stream);
 
+/* ms_invariant_map -- analytic 1-D mappings for invariants (Eq. 15-20): flat (Eq. 20), power law with
+ * exponent nu = par (Eq. 18; par == 1 selects the logarithmic limit Eq. 19; m2 may be the negative auxiliary mass of
+ * PAPER.md:185) and Breit-Wigner with par = m * Gamma (Eq. 16-17).  direction 0: d_out = G(d_in), d_in in [0,1];
+ * direction 1: d_out = G^-1(d_in).  d_g (optional) = density g of Eq. 15 at x.  Bounds: scalars x_min, x_max, or per-event
+ * arrays d_x_min / d_x_max [N] when non-NULL.  MS_EKIN if x_max <= x_min, m Gamma <= 0 or x_min - m2 <= 0 (power law). */
+enum { MS_MAP_FLAT = 0, MS_MAP_POWER = 1, MS_MAP_BW = 2 };
+int ms_invariant_map(int64_t N, int kind, int direction, double x_min, double x_max, const double* d_x_min,
+                     const double* d_x_max, double m2, double par, const double* d_in, double* d_out, double* d_g, void* stream);
+
 /* Observables, cuts and weighted histograms (Sec. 3.2.4-3.2.5; scales Eq. 79-80; the paper names the
  * observables without formulas: DESIGN.md reading O-1).  Particle indices a, b count row blocks: 0, 1 incoming,
  * 2.. outgoing.  phi in (-pi, pi], theta in [0, pi], dphi folded into [0, pi], deta = |eta_a - eta_b|,

@@ -24,7 +24,7 @@ _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECU
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
 
 
 class MadSpaceError(RuntimeError):
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
         L.ms_unweight_scratch_bytes.argtypes = [_i64]
         L.ms_check_grid.argtypes = [_int, _int, _vp]
         L.ms_fill_uniforms.argtypes = [_i64, _int, ms_rng, _vp, _i64, _vp]
+        L.ms_invariant_map.argtypes = [_i64, _int, _int, _dbl, _dbl, _vp, _vp, _dbl, _dbl, _vp, _vp, _vp, _vp]
         L.ms_observable.argtypes = [_i64, _int, _int, _int, _int, _vp, _vp, _i64, _vp]
         L.ms_cut.argtypes = [_i64, _vp, _dbl, _dbl, _vp, _vp]
         L.ms_histogram_fill.argtypes = [_i64, _vp, _vp, _dbl, _dbl, _int, _vp, _vp, _vp]
@@ -314,3 +315,13 @@ def ms_cut(N, d_obs, lo, hi, d_w, stream=None) -> None:
 def ms_histogram_fill(N, d_obs, d_w, lo, hi, n_bins, d_sum_w, d_sum_w2, stream=None) -> None:
     _check("ms_histogram_fill", lib().ms_histogram_fill(N, _ptr(d_obs), _ptr(d_w), float(lo), float(hi), n_bins,
                                                         _ptr(d_sum_w), _ptr(d_sum_w2), _stream(stream)))
+
+
+MAP_KINDS = ("FLAT", "POWER", "BW")
+
+
+def ms_invariant_map(N, kind: str, direction, x_min, x_max, m2, par, d_in, d_out, d_g=None, d_x_min=None, d_x_max=None,
+                     stream=None) -> None:
+    _check("ms_invariant_map", lib().ms_invariant_map(N, MAP_KINDS.index(kind), direction, float(x_min), float(x_max),
+                                                      _ptr(d_x_min), _ptr(d_x_max), float(m2), float(par), _ptr(d_in),
+                                                      _ptr(d_out), _ptr(d_g), _stream(stream)))
