@@ -7,6 +7,7 @@ One step = ms_generate (Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [rescal
 """
 from __future__ import annotations
 
+import contextlib
 from dataclasses import dataclass
 from typing import Optional, Sequence
 
@@ -16,6 +17,19 @@ import torch
 from . import (ms_elementwise_max, ms_weight_histogram, ms_wmax_from_histogram, MS_HIST_BINS,
                ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
                ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID)
+
+
+@contextlib.contextmanager
+def _on(stream):
+    """Make `stream` (a torch.cuda.Stream, a raw cudaStream_t handle, or None = keep the current one) torch's current
+    stream, so that the library calls (which then take the current stream) and the few torch bookkeeping ops between
+    them (zeroing a scalar, allocations) are ordered on ONE stream."""
+    if stream is None:
+        yield
+        return
+    s = stream if isinstance(stream, torch.cuda.Stream) else torch.cuda.ExternalStream(int(stream))
+    with torch.cuda.stream(s):
+        yield
 
 
 @dataclass
@@ -100,37 +114,42 @@ class HotPath:
 
     # ---- stages -------------------------------------------------------------------------------
     def generate(self, event_offset: int = 0, stream=None) -> None:
-        ms_generate(self.cfg, self.N, rng(self.spec.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
-                    self.x1x2, self.ld, self.fail, stream)
+        with _on(stream):
+            ms_generate(self.cfg, self.N, rng(self.spec.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
+                        self.x1x2, self.ld, self.fail, None)
 
     def adapt_grid(self, event_offset: int = 0, alpha: float = 0.5, stream=None) -> np.ndarray:
         """One VEGAS adaptation step from the weights of the last generate(event_offset): accumulate w^2 per bin on the
         device, refine on the host (tiny tables), install the new grid.  Returns the new host edges."""
         if self.d_edges is None:
             raise RuntimeError("adapt_grid needs a grid")
-        hist = torch.zeros((self.grid_dims, self.grid_bins), dtype=torch.float64, device=self.device)
-        ms_vegas_accumulate(self.N, self.grid_dims, self.grid_bins, self.w, rng(self.spec.seed_events, 0, event_offset),
-                            hist, stream)
-        new_edges = ms_vegas_refine(hist.cpu().numpy(), self.d_edges.cpu().numpy(), alpha)
-        self.set_grid(new_edges)
+        with _on(stream):
+            hist = torch.zeros((self.grid_dims, self.grid_bins), dtype=torch.float64, device=self.device)
+            ms_vegas_accumulate(self.N, self.grid_dims, self.grid_bins, self.w, rng(self.spec.seed_events, 0, event_offset),
+                                hist, None)
+            new_edges = ms_vegas_refine(hist.cpu().numpy(), self.d_edges.cpu().numpy(), alpha)
+            self.set_grid(new_edges)
         return new_edges
 
     def unweight(self, event_offset: int = 0, stream=None) -> None:
         s = self.spec
-        self.wmax.zero_()
-        ms_reduce_max(min(s.prerun, self.N), self.w, self.wmax, stream)
-        ms_unweight(self.N, self.w, self.wmax, rng(s.seed_unweight, 1, event_offset), s.rows_p if self.gather_rows else 0,
-                    self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
-                    self.scratch, self.scratch_bytes, self.ld, stream)
+        with _on(stream):
+            self.wmax.zero_()
+            ms_reduce_max(min(s.prerun, self.N), self.w, self.wmax, None)
+            ms_unweight(self.N, self.w, self.wmax, rng(s.seed_unweight, 1, event_offset), s.rows_p if self.gather_rows else 0,
+                        self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
+                        self.scratch, self.scratch_bytes, self.ld, None)
 
     def invert_phase_space(self, stream=None) -> None:
-        ms_fastrambo_inverse(self.N, self.spec.n, self.p, self.x_inv, self.w_inv, self.ld, stream)
+        with _on(stream):
+            ms_fastrambo_inverse(self.N, self.spec.n, self.p, self.x_inv, self.w_inv, self.ld, None)
 
     def invert_grid(self, stream=None) -> None:
         if self.d_edges is not None:
             # only the dimensions the phase-space map consumed are inverted
-            ms_vegas_map(self.N, self.d_inv, self.grid_bins, self.d_edges, 1, self.x_inv, rng(0), self.r_inv, None,
-                         self.ld, stream)
+            with _on(stream):
+                ms_vegas_map(self.N, self.d_inv, self.grid_bins, self.d_edges, 1, self.x_inv, rng(0), self.r_inv, None,
+                             self.ld, None)
 
     def invert(self, stream=None) -> None:
         self.invert_phase_space(stream)
@@ -142,6 +161,21 @@ class HotPath:
             self.unweight(event_offset, stream)
         if self.spec.inverse:
             self.invert(stream)
+
+    def capture(self, event_offset: int = 0) -> "torch.cuda.CUDAGraph":
+        """One step recorded as a CUDA graph (the library calls neither allocate nor synchronise, so a step is
+        capturable as it stands): replay() re-runs it with one launch call, which is what makes sub-wave batches
+        (cfg 1: 2^16 events, 4 kernels of ~5-20 us each) launch-latency-free.  The event offset is baked into the graph:
+        capture one graph per offset in flight, or use step() for varying offsets."""
+        side = torch.cuda.Stream(device=self.device)
+        side.wait_stream(torch.cuda.current_stream(self.device))
+        with torch.cuda.stream(side):
+            self.step(event_offset)                         # warm-up: sets the kernels' shared-memory attributes
+        torch.cuda.current_stream(self.device).wait_stream(side)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            self.step(event_offset)
+        return g
 
     @property
     def launches_per_step(self) -> int:
@@ -170,6 +204,11 @@ class RunningUnweighter:
 
     def add_batch(self, w: torch.Tensor, N: int, event_offset: int, rows: Optional[torch.Tensor] = None, ld: int = 0,
                   stream=None) -> int:
+        with _on(stream):
+            return self._add_batch(w, N, event_offset, rows, ld)
+
+    def _add_batch(self, w, N, event_offset, rows, ld) -> int:
+        stream = None                                        # torch's current stream (set by add_batch)
         ms_weight_histogram(N, w, self.counts, stream)
         self.w_max = max(self.w_max, ms_wmax_from_histogram(self.counts.cpu().numpy(), self.fraction))
         self.trace.append(self.w_max)
@@ -195,6 +234,11 @@ class RunningUnweighter:
 
     def finalize(self, stream=None):
         """Returns (global indices, output weights, rows or None) of the finally unweighted events."""
+        with _on(stream):
+            return self._finalize()
+
+    def _finalize(self):
+        stream = None                                        # torch's current stream (set by finalize)
         f64 = dict(dtype=torch.float64, device=self.device)
         idx_all = torch.cat(self.kept_idx) if self.kept_idx else torch.empty(0, dtype=torch.int64, device=self.device)
         K = idx_all.numel()
