@@ -194,9 +194,23 @@ def time_oracle(wl, target_seconds=12.0, steps=1, warmup=0):
         oracle_step(orc, wl, n)
         times.append(time.perf_counter() - t0)
     t = float(np.mean(times))
-    return {"value": n / t, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "sample": "first %d events (2^%d) of %s per step, %d step(s); OpenMP over event ranges, sequential unweighting"
-                      % (n, n.bit_length() - 1, wl.name, steps)}, t
+    out = {"value": n / t, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+           "sample": "first %d events (2^%d) of %s per step, %d step(s); OpenMP over event ranges, sequential unweighting"
+                     % (n, n.bit_length() - 1, wl.name, steps)}
+    # the same oracle on ONE thread (a per-core figure), on at most 2^20 events
+    try:
+        from threadpoolctl import threadpool_limits
+        n1 = min(n, 1 << 20)
+        with threadpool_limits(limits=1, user_api="openmp"):
+            if orc.num_threads() == 1:
+                t0 = time.perf_counter()
+                oracle_step(orc, wl, n1)
+                out["per_core_value"] = n1 / (time.perf_counter() - t0)
+                out["per_core_sample"] = "first %d events on 1 thread" % n1
+    except Exception as ex:                                   # a reported extra, never a reason to fail the bench
+        out["per_core_value"] = None
+        out["per_core_sample"] = "unavailable: %s" % type(ex).__name__
+    return out, t
 
 
 def run_reference(args):

@@ -59,6 +59,8 @@ typedef struct ms_rng {
 } ms_rng;
 
 const char* ms_version(void);
+/* Raw cudaError_t of the last MS_ECUDA returned to the CALLING THREAD (thread-local; 0 if none). The library keeps no
+ * other state: every call is re-entrant and may be issued from several host threads on different streams. */
 int ms_last_cuda_error(void);
 
 /* Host-side validation of a VEGAS edge table h_edges[d][n_bins+1] (reading V-1):
