@@ -96,7 +96,8 @@ def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
 # (recorded, not measured by this script; --traffic overrides).
-NCU_TRAFFIC = {"cfg2": (3.295168e9 + 62.72e3, "profiles/r01c_cfg2.md")}
+NCU_TRAFFIC = {"cfg2": (3.295350e9 + 513.28e3, "profiles/r01e_final.md"), "cfg3": (16.583720e9 + 112.1e3, "profiles/r01e_final.md"),
+               "cfg5": (5.443808e9 + 91e3, "profiles/r01e_final.md"), "cfg4": (6.651895e9 + 172.5e3, "profiles/r01e_final.md")}
 
 
 def measured_peaks():
@@ -334,6 +335,8 @@ def run_ours(args):
     t_total = ev[0].elapsed_time(ev[1]) * 1e-3
     stage_ms = {name: float(np.mean([m[j].elapsed_time(m[j + 1]) for m in marks])) for j, (name, _) in enumerate(stages)}
     t_gen = stage_ms["generate"] * 1e-3
+    per_step = [m[0].elapsed_time(m[-1]) for m in marks]      # median and best beside the mean
+    step_stats = {"median": float(np.median(per_step)), "best": float(np.min(per_step)), "worst": float(np.max(per_step))}
     n_acc_local = int(hp.n_acc.item()) if wl.unweight else 0
     if world > 1:
         tt = torch.tensor([t_total, t_gen], dtype=torch.float64, device=dev)
@@ -472,7 +475,7 @@ def run_ours(args):
             "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_counter[0],
                     "wall_value": total_events / t_e2e_wall,
                     "what": e2e_what},
-            "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "stage_ms": stage_ms, "cpu_baseline": cb,
+            "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "stage_ms": stage_ms, "ms_per_step_stats": step_stats, "cpu_baseline": cb,
             "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
                             "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
             "fail_count": int(hp.fail.item()),
@@ -480,6 +483,50 @@ def run_ours(args):
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def run_unweight_density(args):
+    """Side measurement (not the bench line): ms_unweight alone on 2^24 synthetic weights x 24 momentum rows at several
+    acceptance rates -- the unweighting efficiencies a production run sees after grid adaptation
+    rather than the 1e-4 of the seeded-grid workloads.  Weights w = u^(1/f - 1) with w_max = 1 have <w>/w_max = f."""
+    import torch
+    import paper_2602_06895_b200 as ms
+    ms.lib()
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    N, rows = 1 << 24, 24
+    f64 = dict(dtype=torch.float64, device=dev)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(5)
+    p = torch.rand((rows, N), generator=gen, **f64)
+    idx = torch.empty(N, dtype=torch.int64, device=dev)
+    w_out, rows_out = torch.empty(N, **f64), torch.empty((rows, N), **f64)
+    n_acc = torch.zeros(1, dtype=torch.int64, device=dev)
+    sb = ms.ms_unweight_scratch_bytes(N)
+    scratch = torch.empty(sb, dtype=torch.uint8, device=dev)
+    wmax = torch.ones(1, **f64)
+    out = []
+    for frac in (1e-4, 1e-3, 1e-2, 0.1, 0.5, 1.0):
+        w = torch.rand(N, generator=gen, **f64) ** (1.0 / frac - 1.0)
+
+        def call():
+            ms.ms_unweight(N, w, wmax, ms.rng(ms_inputs.SEED_UNWEIGHT, 1, 0), rows, p, N, idx, w_out, rows_out, n_acc, scratch,
+                           sb, N, None)
+        for _ in range(max(args.warmup, 3)):
+            call()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(args.steps):
+            call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        us = ev[0].elapsed_time(ev[1]) * 1e3 / args.steps
+        k = int(n_acc.item())
+        moved = 8 * N + k * 16 * (rows + 2)                    # weights read + (idx, w_out, rows) read and written
+        out.append({"efficiency": frac, "accepted": k, "us_per_call": us, "algorithmic_gb_per_s": moved / us / 1e3})
+    print(json.dumps({"probe": "unweight-density", "events": N, "rows": rows, "steps": args.steps, "results": out}))
     return 0
 
 
@@ -493,7 +540,12 @@ def main():
     ap.add_argument("--events", type=int, default=0, help="override events per GPU per step (0 = the workload's)")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: do not time the oracle")
     ap.add_argument("--traffic", type=float, default=0.0, help="dram bytes per launch of the dominant kernel from ncu (recorded, not measured here)")
+    ap.add_argument("--probe", default="", choices=["", "unweight-density"],
+                    help="side measurements for DESIGN.md / profiles (not the bench line)")
     args = ap.parse_args()
+    if args.probe == "unweight-density":
+        args.steps = min(args.steps, 20)
+        return run_unweight_density(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
