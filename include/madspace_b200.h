@@ -76,8 +76,12 @@ int ms_check_grid(int d, int n_bins, const double* h_edges);
  *       own path through a breadth-first edge tree in shared memory), r = (j + (x-x_j)/(x_{j+1}-x_j))/n_bins;
  *       d_jac[e] = 1/prod(...).
  *       d_in = x rows (must not be NULL).
+ *       The quotient is the IEEE-754 correctly rounded one (the divisor-only part of div.rn.f64 is tabulated per
+ *       bin; inputs outside its fast path go through div.rn.f64 itself): results are bit-identical to a / b on the host.
  * d_edges: device table [d][n_bins+1], validated by the caller with ms_check_grid.
- * d_out: [d][ld].  d_jac: [N] or NULL.  d_in and d_out may alias. */
+ * d_out: [d][ld].  d_jac: [N] or NULL.  d_in and d_out may alias.
+ * Errors: MS_EINVAL on bad sizes or pointers, or if the tables exceed 200 KB of shared memory
+ * (forward: 16 d n_bins bytes; inverse: 16 d (n_bins+1) + 4 d 2^ceil(log2 n_bins) bytes). */
 int ms_vegas_map(int64_t N, int d, int n_bins, const double* d_edges, int direction,
                  const double* d_in, ms_rng rng, double* d_out, double* d_jac, int64_t ld, void* stream);
 
