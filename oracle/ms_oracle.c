@@ -18,8 +18,8 @@
  * unit VEGAS Jacobian / identity on uniform grids; forward o inverse round trips;
  * Table 1 re-fit from Eq. 66; massive two-body closed form and nested-quadrature
  * massive volume; literal __float128 transcription (ms_oracle_lit.c).
- * Parity unpinned: absolute normalisation of the toy integrand (not from the paper;
- * it has no closed form) -- see DESIGN.md.
+ * Parity unpinned: nothing (the toy integrand, not from the paper, is pinned by brute force at every n,
+ * by the closed form at n = 2 and by the Dalitz-plot quadrature of its cross-section at n = 3: tests/).
  *
  * Layout convention (an interface, not shared code): structure of arrays,
  * a[row*ld + e] for event e; momentum row = 4*particle + mu, mu = (E,px,py,pz)

@@ -314,6 +314,32 @@ def test_toy_integrand_bruteforce(orc):
     assert np.max(np.abs(orc.toy_integrand(n, p2) / f - 1)) < 1e-14
 
 
+def test_toy_cross_section_three_body_dalitz(orc):
+    """Absolute normalisation of the weighted toy integrand at n = 3, against a number the oracle has no part in:
+    for massless particles s_ij = 2 p_i.p_j, and the three-body phase space in Dalitz variables is
+    dPhi_3 = ds_12 ds_23 / (128 pi^3 s) on the triangle s_12 + s_23 <= s (PDG kinematics; its area s^2/2 reproduces
+    Eq. 81's Phi_3 = s / (256 pi^3)), so
+        int dPhi_3 f = 1/(128 pi^3 s) int_0^s dx ln((s - x + a)/a) / (x + a),     f = 1/((s_12+a)(s_23+a)),
+    a one-dimensional quadrature typed out here.  <w f> from FastRambo and from the exact Rambo chain must both hit it."""
+    W = 1000.0
+    s = W * W
+    assert abs(orc.phi_n(3, W) / (s / (256 * math.pi ** 3)) - 1) < 1e-14
+    N = 1 << 22
+    x = orc.fill_uniforms(N, 5, 17)
+    # a = (250 GeV)^2: smooth integrand, per-mille Monte Carlo error -- a wrong factor 2, pi or pair cannot hide;
+    # a = TOY_REG = (10 GeV)^2, the benchmark's regulator: peaked (f spans 10^8), the same check at its 5 % error
+    for a, max_rel_err in ((62500.0, 1.5e-3), (ms_inputs.TOY_REG, 8e-2)):
+        inner = lambda t: math.log((s - t + a) / a) / (t + a)
+        ref = integrate.quad(inner, 0.0, s, epsabs=0, epsrel=1e-12, points=[10 * a, min(1000 * a, 0.5 * s)], limit=400)[0]
+        ref /= 128 * math.pi ** 3 * s
+        for fn in (orc.fastrambo, orc.rambo_massless):
+            p, w = fn(3, x, W)
+            wf = w * orc.toy_integrand(3, p, a)
+            err = wf.std() / math.sqrt(N)
+            assert err / ref < max_rel_err, (a, err / ref)
+            assert abs(wf.mean() - ref) < 5 * err, (a, wf.mean(), ref, err)
+
+
 # ------------------------------------------------------------ unweighting
 
 def test_unweight_bruteforce_and_sum_identity(orc):
