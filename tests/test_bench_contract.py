@@ -1,4 +1,4 @@
-"""bench.py's contract, as far as it can be checked without a GPU: the reference arm (the oracle timed on the host cores)
+"""bench.py's contract, the reference arm (the oracle timed on the host cores)
 prints ONE JSON line with the keys the driver reads, non-zero ranks of a multi-process launch print nothing, and the
 hand-counted roofline inputs (algorithmic bytes and fp64 instructions per event) follow the workload definitions."""
 import json
@@ -51,3 +51,28 @@ def test_roofline_inputs_follow_the_workloads():
     # the hand count grows with the multiplicity and with every optional stage
     c = {k: bench.alg_fp64_per_event(ms_inputs.WORKLOADS[k]) for k in ms_inputs.WORKLOADS}
     assert c["cfg1"] < c["cfg2"] < c["cfg5"] and c["cfg4rw"] < c["cfg4"]
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_our_arm_prints_one_contract_line_on_the_gpu():
+    """The product arm on a reduced event count (the full-size line is the driver's to take): every key of the contract
+    is there, the launch count is the library's own kernels, and the e2e leg really moved bytes both ways."""
+    out = run_bench("--steps", "3", "--warmup", "3", "--events", str(1 << 20), "--skip-cpu-baseline").strip().splitlines()
+    assert len(out) == 1
+    d = json.loads(out[0])
+    assert "impl" not in d or d["impl"] != "reference"
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["steps"] == 3 and d["warmup"] == 3 and d["n_gpus"] == 1 and d["scaling"] == "weak" and d["dtype"] == "f64"
+    assert d["gpu_launches"] == 4 * 3                      # generate, reduce_max, decide, scatter per step
+    r = d["roofline"]
+    assert r["bound"] in ("hbm", "alu") and r["unit"].split()[0] in ("GB/s", "Ginst/s") and r["peak"] > 0
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0 < r["frac"] < 1.0
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    assert d["fail_count"] == 0 and d["unweighted"]["accepted_per_step_per_rank"][0] > 0
+    assert "sm_mhz" in d["clocks"] and "reasons" in d["clocks"]
