@@ -344,6 +344,7 @@ def run_ours(args):
         t_total, t_gen = float(tt[0]), float(tt[1])
     counts = gather_counts(n_acc_local)
     offsets = output_offsets(counts)
+    launches_all = sum(gather_counts(hp.launches(offset) * args.steps))   # ranks > 0 replay the pre-run: one more launch
 
     # ---- end to end through the public API with HOST buffers: every step copies its input (the grid table) from pinned
     # host memory and the host reads the step's result.  For a generator the result is the unweighted sample: the
@@ -475,7 +476,7 @@ def run_ours(args):
             "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_counter[0],
                     "wall_value": total_events / t_e2e_wall,
                     "what": e2e_what},
-            "gpu_launches": hp.launches_per_step * args.steps, "roofline": roof, "stage_ms": stage_ms, "ms_per_step_stats": step_stats, "cpu_baseline": cb,
+            "gpu_launches": launches_all, "roofline": roof, "stage_ms": stage_ms, "ms_per_step_stats": step_stats, "cpu_baseline": cb,
             "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
                             "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
             "fail_count": int(hp.fail.item()),

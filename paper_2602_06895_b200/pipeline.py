@@ -91,6 +91,8 @@ class HotPath:
             self.n_acc = torch.zeros(1, dtype=torch.int64, device=self.device)
             self.scratch_bytes = ms_unweight_scratch_bytes(self.N)
             self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
+            self._pre = None                                   # buffers of the replayed pre-run, allocated on first use
+            self.fail_pre = torch.zeros(1, dtype=torch.int32, device=self.device)
         if spec.inverse:
             self.d_inv = 3 * spec.n - 4
             self.x_inv = torch.empty((self.d_inv, self.ld), **f64)
@@ -135,7 +137,20 @@ class HotPath:
         s = self.spec
         with _on(stream):
             self.wmax.zero_()
-            ms_reduce_max(min(s.prerun, self.N), self.w, self.wmax, None)
+            if event_offset == 0 and self.N >= s.prerun:
+                ms_reduce_max(s.prerun, self.w, self.wmax, None)    # the batch starts with the pre-run events
+            else:
+                # w_max is the maximum over the GLOBAL events 0..prerun-1 (reading R-4), whatever range this batch or
+                # this rank owns: replay them (deterministic, no communication)
+                if self._pre is None:
+                    ld = (s.prerun + 1) // 2 * 2
+                    f64 = dict(dtype=torch.float64, device=self.device)
+                    self._pre = (torch.empty((s.rows_p, ld), **f64), torch.empty(ld, **f64),
+                                 torch.empty((2, ld), **f64) if s.pdf else None, ld)
+                p_pre, w_pre, x_pre, ld = self._pre
+                ms_generate(self.cfg, s.prerun, rng(s.seed_events, 0, 0), self.d_edges, p_pre, w_pre, x_pre, ld,
+                            self.fail_pre, None)
+                ms_reduce_max(s.prerun, w_pre, self.wmax, None)
             ms_unweight(self.N, self.w, self.wmax, rng(s.seed_unweight, 1, event_offset), s.rows_p if self.gather_rows else 0,
                         self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
                         self.scratch, self.scratch_bytes, self.ld, None)
@@ -177,15 +192,20 @@ class HotPath:
             self.step(event_offset)
         return g
 
-    @property
-    def launches_per_step(self) -> int:
-        """Kernels of this library enqueued by one step() (memsets/copies not counted)."""
+    def launches(self, event_offset: int = 0) -> int:
+        """Kernels of this library enqueued by one step(event_offset) (memsets/copies not counted)."""
         k = 1
         if self.spec.unweight:
             k += 3                                  # ms_reduce_max + decide / scatter of ms_unweight
+            if not (event_offset == 0 and self.N >= self.spec.prerun):
+                k += 1                              # the replayed pre-run (ms_generate over events 0..prerun-1)
         if self.spec.inverse:
             k += 2 if self.d_edges is not None else 1
         return k
+
+    @property
+    def launches_per_step(self) -> int:
+        return self.launches(0)
 
 
 class RunningUnweighter:
