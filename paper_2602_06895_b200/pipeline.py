@@ -133,10 +133,11 @@ class HotPath:
             self.set_grid(new_edges)
         return new_edges
 
-    def unweight(self, event_offset: int = 0, stream=None) -> None:
+    def unweight(self, event_offset: int = 0, stream=None, _wmax_zeroed: bool = False) -> None:
         s = self.spec
         with _on(stream):
-            self.wmax.zero_()
+            if not _wmax_zeroed:
+                self.wmax.zero_()
             if event_offset == 0 and self.N >= s.prerun:
                 ms_reduce_max(s.prerun, self.w, self.wmax, None)    # the batch starts with the pre-run events
             else:
@@ -171,9 +172,14 @@ class HotPath:
         self.invert_grid(stream)
 
     def step(self, event_offset: int = 0, stream=None) -> None:
+        if self.spec.unweight:
+            # w_max is zeroed BEFORE the generation kernel, so that ms_reduce_max follows it directly in the stream and
+            # its programmatic dependent launch overlaps the generation kernel's tail
+            with _on(stream):
+                self.wmax.zero_()
         self.generate(event_offset, stream)
         if self.spec.unweight:
-            self.unweight(event_offset, stream)
+            self.unweight(event_offset, stream, _wmax_zeroed=True)
         if self.spec.inverse:
             self.invert(stream)
 
