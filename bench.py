@@ -6,9 +6,12 @@
 A step = one pass of the whole hot path over one batch of synthetic (Philox-seeded) events: for the default
 workload (BASELINE.json configs[1], "cfg2": massless 2->4 FastRambo, 2^24 events, seeded 128x8 VEGAS grid, toy
 integrand, unweighting) that is ms_generate -> ms_reduce_max (pre-run w_max) -> ms_unweight.
-N > 1 (torchrun): one process per GPU, every rank generates its own 2^24-event batch at event offset rank*2^24
-(weak scaling, no data-path collective); value = events of all ranks / max-over-ranks time.
---impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+Consecutive steps continue the event stream (step k of rank g starts at event (k*G + g)*2^24), as a generator does;
+w_max of the 2^16-event pre-run is a function of (spec, grid) and is computed once, by the first warm-up step.
+N > 1 (torchrun): one process per GPU (weak scaling, no data-path collective); value = events of all
+ranks / max-over-ranks time.  --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the
+same workload.  At N = 1 the same run also measures the other BASELINE.json configs (`per_config`: every stage with its
+own roofline, sampled parity against the oracle, Monte Carlo mean against the closed forms of BASELINE.md section 2).
 """
 from __future__ import annotations
 
@@ -72,6 +75,28 @@ ALG_FP64 = {"uniform": 1, "vegas_dim": 5, "decay_first": 3 + SQRT + 1 + SINCOS +
 RESCALE_EVALUATIONS = 4    # cfg4 converges in <= 3 Newton steps: 4 evaluations of F
 
 
+def alg_bytes_per_event(wl: ms_inputs.Workload) -> int:
+    """Bytes one event must move with everything fused: its output rows (+ the x1, x2 rows where Bjorken x are sampled)."""
+    return wl.out_bytes_per_event + (16 if wl.pdf else 0)
+
+
+def alg_fp64_inverse(n: int) -> int:
+    """FastRambo inverse (ms_kernels.cuh inverse_kernel), hand count per event: per decay the suffix sum (4), Q^2 (4),
+    floor + max (3), sqrt with 1/(2M) (7), 1/M (1), rest-frame energy (5), boost factor (2 + RCP), three components (3),
+    |p| (3 + 1 + 7), cos theta (1), azimuth (24: octant folding, one reciprocal, degree-11 polynomial); per mass step
+    u, y = u^(2k), 1 - y, D (2), Eq. 64 (3 + RCP), 1 - u^2, two weight products (8)."""
+    per_decay = 4 + 4 + 3 + SQRT_H + 1 + 5 + 2 + RCP + 3 + 3 + 1 + SQRT_H + 1 + 24
+    c = (n - 1) * per_decay
+    for i in range(2, n):
+        k = n - i
+        c += 1 + _pow_cost(2 * k) + 1 + 2 + 3 + RCP + 1 + 8
+    return c + 4 + RCP
+
+
+VEGAS_INVERSE_FP64_PER_VALUE = 8       # two subtractions, three-instruction quotient, j + q, / n_bins, one comparison
+PHILOX_IMAD_WIDE = 20                  # 32x32 -> 64-bit multiplies per Philox4x32-10 call (one per unweighting decision)
+
+
 def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
     n = wl.n
     c = ALG_FP64["uniform"] * wl.d + ALG_FP64["vegas_dim"] * wl.grid_dims
@@ -94,10 +119,22 @@ def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
     return c + ALG_FP64["weight"]
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
-# (recorded, not measured by this script; --traffic overrides).
-NCU_TRAFFIC = {"cfg2": (3.295350e9 + 513.28e3, "profiles/r01e_final.md"), "cfg3": (16.583720e9 + 112.1e3, "profiles/r01e_final.md"),
-               "cfg5": (5.443808e9 + 91e3, "profiles/r01e_final.md"), "cfg4": (6.651895e9 + 172.5e3, "profiles/r01e_final.md")}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu captures (recorded, not measured by
+# this script; --traffic overrides the headline's): {workload: {stage: (bytes, source)}}.
+NCU_TRAFFIC = {
+    "cfg2": {"generate": (3.295350e9 + 513.28e3, "profiles/r01e_final.md"), "unweight": (134.25e6 + 3.9e6 + 7.7e6, "profiles/r01e_final.md")},
+    "cfg3": {"generate": (16.583720e9 + 112.1e3, "profiles/r01e_final.md")},
+    "cfg4": {"generate": (6.651895e9 + 172.5e3, "profiles/r01e_final.md")},
+    "cfg5": {"generate": (5.443808e9 + 91e3, "profiles/r01e_final.md"), "vegas_inverse": (2.684e9 + 2.638e9, "profiles/r01e_final.md")},
+}
+
+# Closed forms of BASELINE.md section 2 (Eq. 81 and the quadratures pinned in tests/test_oracle_phasespace.py): what the
+# Monte Carlo mean of the phase-space weights (toy integrand off) must converge to.
+CLOSED_FORM = {"cfg1": (125.982556379686, "Phi_3(1000 GeV), Eq. 81"), "cfg2": (132965.643027888, "Phi_4(1000 GeV), Eq. 81"),
+               "cfg3": (2.77492935789908e13, "Phi_5(1) s_had^3 [(1-tau_min^4)/16 + tau_min^4 ln(tau_min)/4]"),
+               "cfg4": (1500880.28692, "Phi_4(2000 GeV; 173,173,0,0), nested two-body quadrature"),
+               "cfg4rw": (1500880.28692, "Phi_4(2000 GeV; 173,173,0,0), nested two-body quadrature"),
+               "cfg5": (3.75780115705882e20, "Phi_8(3000 GeV), Eq. 81")}
 
 
 def measured_peaks():
@@ -177,7 +214,7 @@ def oracle_step(orc, wl, n_events, offset=0):
     return n_acc
 
 
-def time_oracle(wl, target_seconds=12.0, steps=1, warmup=0):
+def time_oracle(wl, target_seconds=12.0, steps=1, warmup=0, per_core=True):
     import oracle as orc
     orc.lib()
     probe = 1 << 16
@@ -198,6 +235,8 @@ def time_oracle(wl, target_seconds=12.0, steps=1, warmup=0):
     out = {"value": n / t, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
            "sample": "first %d events (2^%d) of %s per step, %d step(s); OpenMP over event ranges, sequential unweighting"
                      % (n, n.bit_length() - 1, wl.name, steps)}
+    if not per_core:
+        return out, t
     # the same oracle on ONE thread (a per-core figure), on at most 2^20 events
     try:
         from threadpoolctl import threadpool_limits
@@ -233,6 +272,8 @@ def run_reference(args):
 def workload_config(wl, n_gpus):
     return {"workload": "%s: %s" % (wl.name, wl.note), "events_per_gpu_per_step": wl.N, "n": wl.n,
             "grid": "%dx%d %s" % (wl.grid_bins, wl.grid_dims, wl.grid_kind), "parallelism": "events sharded x%d" % n_gpus,
+            "offsets": "step k of rank g generates events [(k*G+g)*N, (k*G+g+1)*N) of the Philox stream",
+            "wmax": "max weight of the 2^16-event pre-run (events 0..65535): a function of (spec, grid), computed once by the first warm-up step",
             "l2": "no flush needed: each step streams %.2f GB of fresh output (> 126 MB L2)" % (wl.N * wl.out_bytes_per_event / 1e9)}
 
 
@@ -247,39 +288,191 @@ def spec_from_workload(wl):
                     seed_unweight=ms_inputs.SEED_UNWEIGHT)
 
 
-def probe_fp64_rate(ms, torch, seconds=0.25, three_regs=False):
-    """Sustained DFMA issue rate (instructions/s) measured with ms_probe_dfma (register * constant + constant) or
-    ms_probe_dfma3 (three distinct register operands): 8 independent chains per thread."""
-    probe = ms.ms_probe_dfma3 if three_regs else ms.ms_probe_dfma
-    sms = torch.cuda.get_device_properties(0).multi_processor_count
-    blocks, iters = sms * 8, 1 << 14
-    sink = torch.empty(blocks * 256, dtype=torch.float64, device="cuda")
-    probe(blocks, iters, sink)
-    torch.cuda.synchronize()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps, best, t_end = 0, 0.0, time.perf_counter() + seconds
-    while time.perf_counter() < t_end or reps < 3:
-        ev0.record()
-        probe(blocks, iters, sink)
-        ev1.record()
-        ev1.synchronize()
-        best = max(best, blocks * 256 * iters * 8 / (ev0.elapsed_time(ev1) * 1e-3))
-        reps += 1
-    return best
+def measure_peaks(torch, sms):
+    """The roofline denominators: HBM from MEASURED_PEAKS.json (driver-written), the fp64 pipe MEASURED here (SURVEY.md
+    section 8d: a dependent-free DFMA loop sustained for seconds; the median launch is the denominator), the quarter-rate
+    32x32->64 multiply pipe of Philox measured the same way."""
+    import bench_probes
+    hbm_gbs, sm_max_mhz, src = measured_peaks()
+    dfma = bench_probes.fp64_rate(torch, 2.0)
+    dfma3 = bench_probes.fp64_rate(torch, 1.0, three_regs=True)
+    imad = bench_probes.imad_wide_rate(torch)
+    return {"hbm_gbs": hbm_gbs, "hbm_source": src, "sm_max_mhz": sm_max_mhz,
+            "fp64_ginst_nominal": sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6 / 1e9,
+            "fp64_ginst_measured": dfma["median"] / 1e9, "fp64_ginst_measured_best": dfma["best"] / 1e9,
+            "fp64_probe": "8 independent DFMA chains per thread, %d launches over >= %.0f s, median" % (dfma["launches"], dfma["seconds"]),
+            "fp64_ginst_3reg_operands": dfma3["median"] / 1e9, "imad_wide_ginst_measured": imad / 1e9}
 
 
-def probe_write_stream(ms, torch, hp, wl, reps=10):
-    """GB/s of the generation kernel's store pattern with no arithmetic (ms_probe_write into the momentum buffer)."""
-    rows = hp.spec.rows_p
-    ms.ms_probe_write(hp.N, rows, hp.p, hp.ld)
+def stage_roofline(name, wl, N, t_ms, peaks, n_accepted=0, d_inv=0, traffic=None):
+    """Roofline of one stage: time = max over the sides that can bind it; frac = that time / measured time."""
+    hbm, fp64 = peaks["hbm_gbs"] * 1e9, peaks["fp64_ginst_measured"] * 1e9
+    rows_p = 4 * (wl.n + 2)
+    sides = {}
+    if name == "generate":
+        nbytes, ninst = N * alg_bytes_per_event(wl), N * alg_fp64_per_event(wl)
+        sides = {"hbm": nbytes / hbm, "alu": ninst / fp64}
+        extra = {"alg_bytes_per_event": alg_bytes_per_event(wl), "alg_fp64_inst_per_event": alg_fp64_per_event(wl),
+                 "kernel": "ms::gen_kernel<%d,%s,%s%s%s%s>" % (wl.n, "exact" if wl.mapping == "rambo" else "fast",
+                                                             ("rescale" if wl.massive_mode == "rescale" else "reweight") if wl.masses else "massless",
+                                                             ",pdf" if wl.pdf else "", ",toy" if wl.toy else "", ",grid" if wl.grid_dims else "")}
+    elif name == "unweight":
+        nbytes = 8 * N + n_accepted * 16 * (rows_p + 2)
+        sides = {"hbm": nbytes / hbm, "imad": N * PHILOX_IMAD_WIDE / (peaks["imad_wide_ginst_measured"] * 1e9)}
+        extra = {"alg_bytes": nbytes, "alg_imad_wide_per_event": PHILOX_IMAD_WIDE,
+                 "kernel": "ms::unweight_decide_kernel + ms::unweight_scatter_kernel",
+                 "note": "SURVEY 8(d)'s 8 B/event read stream, and the quarter-rate integer-multiply pipe of the one Philox call "
+                         "per decision (20 IMAD.WIDE): the larger of the two is the ceiling"}
+    elif name == "fastrambo_inverse":
+        nbytes = N * (32 * wl.n + 8 * d_inv + 8)
+        sides = {"hbm": nbytes / hbm, "alu": N * alg_fp64_inverse(wl.n) / fp64}
+        extra = {"alg_bytes_per_event": 32 * wl.n + 8 * d_inv + 8, "alg_fp64_inst_per_event": alg_fp64_inverse(wl.n),
+                 "kernel": "ms::inverse_kernel<%d>" % wl.n}
+    elif name == "vegas_inverse":
+        nbytes = N * 16 * d_inv
+        sides = {"hbm": nbytes / hbm, "alu": N * d_inv * VEGAS_INVERSE_FP64_PER_VALUE / fp64}
+        extra = {"alg_bytes_per_event": 16 * d_inv, "kernel": "ms::vegas_inverse_kernel"}
+    else:
+        return None
+    bound = max(sides, key=sides.get)
+    t_roof = sides[bound]
+    out = {"ms": t_ms, "bound": bound, "roofline_ms": 1e3 * t_roof, "frac": 1e3 * t_roof / t_ms if t_ms > 0 else None,
+           "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None}
+    out.update({"%s_time_ms" % k: 1e3 * v for k, v in sides.items()})
+    out.update(extra)
+    return out
+
+
+def time_steps(torch, hp, steps, warmup, first_offset, stride, barrier):
+    """W warm-up steps, then exactly K steps between barriers, every stage bracketed by CUDA events on the launching
+    stream.  Returns total seconds, mean ms per stage, per-step ms list, the offset after the last step."""
+    stream = torch.cuda.current_stream()
+    off = first_offset
+    for _ in range(warmup):
+        hp.step(off)
+        off += stride
+    barrier()
+    stages = hp.stages()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    marks = [[torch.cuda.Event(enable_timing=True) for _ in range(len(stages) + 1)] for _ in range(steps)]
+    ev[0].record(stream)
+    for k in range(steps):
+        marks[k][0].record(stream)
+        for j, (_, fn) in enumerate(stages):
+            fn(off)
+            marks[k][j + 1].record(stream)
+        off += stride
+    ev[1].record(stream)
+    barrier()
+    t_total = ev[0].elapsed_time(ev[1]) * 1e-3
+    stage_ms = {name: float(np.mean([m[j].elapsed_time(m[j + 1]) for m in marks])) for j, (name, _) in enumerate(stages)}
+    per_step = [m[0].elapsed_time(m[-1]) for m in marks]
+    return t_total, stage_ms, per_step, off
+
+
+def sample_indices(N, seed=11, n_random=2048):
+    rs = np.random.Generator(np.random.Philox(key=seed))
+    parts = [np.arange(0, min(256, N)), np.arange(max(N - 256, 0), N), rs.integers(0, N, n_random)]
+    return np.unique(np.concatenate(parts)).astype(np.int64)
+
+
+def parity_and_pins(torch, ms, hp, wl, name):
+    """BASELINE.md section 4, per config: max parity deviations against the oracle on sampled events of a batch at offset 0
+    (the launch configuration just timed), the round trip over EVERY value (cfg 5), and the Monte Carlo mean of the
+    phase-space weights against the closed form (toy integrand off: one more launch of the same kernel family)."""
+    import oracle as orc
+    from oracle.chain import oracle_chain
+    from paper_2602_06895_b200.pipeline import HotPath
+    orc.lib()
+    N, n, dev = hp.N, wl.n, hp.device
+    hp.step(0)
     torch.cuda.synchronize()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    for _ in range(reps):
-        ms.ms_probe_write(hp.N, rows, hp.p, hp.ld)
-    ev1.record()
-    ev1.synchronize()
-    return 8.0 * rows * hp.N * reps / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
+    idx = sample_indices(N)
+    t_idx = torch.from_numpy(idx).to(dev)
+    p = hp.p[:, t_idx].cpu().numpy()
+    w = hp.w[t_idx].cpu().numpy()
+    ref = oracle_chain(orc, wl, idx)
+    rel = np.abs(w - ref["w"]) / ref["w"]
+    out = {"sampled_events": int(idx.size), "max_dp_over_sqrt_s": float(np.max(np.abs(p - ref["p"])) / wl.sqrt_s),
+           "max_rel_dw": float(rel.max()), "n_rel_dw_above_1e-12": int((rel > 1e-12).sum()), "fail_count": int(hp.fail.item())}
+    if wl.unweight:
+        w_all = np.ascontiguousarray(hp.w[:N].cpu().numpy())
+        wmax = float(hp.wmax.item())
+        idx_o, wout_o, nacc_o = orc.unweight(w_all, wmax, ms_inputs.SEED_UNWEIGHT, ms_inputs.STREAM_UNWEIGHT, 0, N)
+        k = int(hp.n_acc.item())
+        out["unweighting_bit_exact_vs_oracle_on_all_weights"] = bool(
+            k == nacc_o and np.array_equal(hp.idx[:k].cpu().numpy(), idx_o) and np.array_equal(hp.w_out[:k].cpu().numpy(), wout_o))
+        out["accepted"] = k
+        out["unweighting_efficiency"] = float(w_all.mean() / wmax)
+        del w_all
+    if wl.inverse:
+        d = 3 * n - 4
+        r = torch.empty((d, hp.ld), dtype=torch.float64, device=dev)
+        ms.ms_fill_uniforms(N, d, ms.rng(ms_inputs.SEED_EVENTS, 0, 0), r, hp.ld)
+        dr = (hp.r_inv[:, :N] - r[:, :N]).abs_()
+        phi_rows = torch.tensor([n - 1 + 2 * a for a in range(n - 1)], device=dev)
+        dr[phi_rows] = torch.minimum(dr[phi_rows], 1.0 - dr[phi_rows])          # the azimuth is periodic
+        worst = dr.amax(dim=0)
+        out["round_trip"] = {"values": int(N) * d, "median_abs_dr": float(dr.flatten()[::16].median()),
+                             "max_abs_dr": float(worst.max()), "events_with_dr_above_1e-10": int((worst > 1e-10).sum()),
+                             "note": "r -> VEGAS -> FastRambo -> inverse -> VEGAS^-1 -> r'; the tail is reading F-7 (information lost at "
+                                     "the fp64 store of near-collinear last pairs, divided by bins as narrow as 1e-6)"}
+        del r, dr, worst
+    # Monte Carlo mean of jac * w_PS [* J_x] [* w_m] against the closed form
+    closed, what = CLOSED_FORM[name]
+    if wl.toy:
+        import dataclasses
+        spec = spec_from_workload(dataclasses.replace(wl, toy=False, unweight=False, inverse=False))
+        h2 = HotPath(spec, N, dev)
+        h2.generate(0)
+        wv = h2.w[:N]
+    else:
+        wv = hp.w[:N]
+    mean, std = float(wv.mean()), float(wv.std())
+    out["mc_mean_over_closed_form"] = {"ratio": mean / closed, "mc_error": std / np.sqrt(N) / closed, "closed_form": closed,
+                                       "what": what, "events": int(N)}
+    return out
+
+
+def measure_config(torch, ms, name, steps, warmup, peaks, oracle_seconds):
+    from paper_2602_06895_b200.pipeline import HotPath
+    wl = ms_inputs.WORKLOADS[name]
+    N = wl.N
+    hp = HotPath(spec_from_workload(wl), N, "cuda:%d" % torch.cuda.current_device(), cap=max(1 << 16, N // 256))
+    t_total, stage_ms, per_step, _ = time_steps(torch, hp, steps, warmup, 0, N, torch.cuda.synchronize)
+    n_acc = int(hp.n_acc.item()) if wl.unweight else 0
+    d_inv = 3 * wl.n - 4
+    traffic = NCU_TRAFFIC.get(name, {})
+    stages = {k: stage_roofline(k, wl, N, v, peaks, n_acc, d_inv, traffic.get(k)) for k, v in stage_ms.items()}
+    out = {"workload": "%s: %s" % (name, wl.note), "events_per_step": N, "steps": steps, "warmup": warmup,
+           "ms_per_step": 1e3 * t_total / steps, "events_per_s": N * steps / t_total,
+           "ms_per_step_median": float(np.median(per_step)), "stages": stages}
+    g = stages["generate"]
+    out.update(kernel=g["kernel"], kernel_ms=g["ms"], bound=g["bound"], frac=g["frac"], hbm_time_ms=g["hbm_time_ms"],
+               alu_time_ms=g["alu_time_ms"], alg_bytes_per_event=g["alg_bytes_per_event"],
+               alg_fp64_inst_per_event=g["alg_fp64_inst_per_event"], traffic=g["traffic"])
+    if N < (1 << 20):
+        # sub-wave batch (cfg 1: 2^16 events = 256 of the >= 1184 resident blocks): launch-latency bound; the number that
+        # matters is the step replayed from a CUDA graph
+        g_ = hp.capture(0)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record()
+        for _ in range(200):
+            g_.replay()
+        ev[1].record()
+        torch.cuda.synchronize()
+        out["cuda_graph_replay_ms_per_step"] = ev[0].elapsed_time(ev[1]) / 200
+        out["note"] = "sub-wave batch: launch-latency bound, reported, not a roofline target"
+    if wl.unweight:
+        out["unweighted_events_per_s"] = n_acc * steps / t_total
+    out["parity"] = parity_and_pins(torch, ms, hp, wl, name)
+    if oracle_seconds > 0:
+        cb, _ = time_oracle(wl, target_seconds=oracle_seconds, per_core=False)
+        out["cpu_baseline"] = cb
+    del hp
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_ours(args):
@@ -288,7 +481,7 @@ def run_ours(args):
 
     import paper_2602_06895_b200 as ms
     from paper_2602_06895_b200.pipeline import HotPath
-    from paper_2602_06895_b200.sharding import gather_counts, output_offsets, weak_range
+    from paper_2602_06895_b200.sharding import gather_counts, output_offsets
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference for the oracle)")
@@ -301,10 +494,10 @@ def run_ours(args):
     ms.lib()
     wl = ms_inputs.WORKLOADS[args.workload]
     N = wl.N if args.events <= 0 else args.events
-    offset, _ = weak_range(N, rank)
     dev = torch.device("cuda", local)
     hp = HotPath(spec_from_workload(wl), N, dev, cap=max(1 << 16, N // 256))
     stream = torch.cuda.current_stream()
+    first_offset, stride = rank * N, world * N          # step k of rank g: events [(k*G+g)*N, (k*G+g+1)*N)
 
     def barrier():
         if world > 1:
@@ -312,30 +505,9 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps between barriers + synchronize
-    for _ in range(args.warmup):
-        hp.step(offset)
-    barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    stages = [("generate", lambda: hp.generate(offset))]
-    if wl.unweight:
-        stages.append(("unweight", lambda: hp.unweight(offset)))
-    if wl.inverse:
-        stages.append(("fastrambo_inverse", hp.invert_phase_space))
-        stages.append(("vegas_inverse", hp.invert_grid))
-    marks = [[torch.cuda.Event(enable_timing=True) for _ in range(len(stages) + 1)] for _ in range(args.steps)]
-    ev[0].record(stream)
-    for k in range(args.steps):
-        marks[k][0].record(stream)
-        for j, (_, fn) in enumerate(stages):
-            fn()
-            marks[k][j + 1].record(stream)
-    ev[1].record(stream)
-    barrier()
-    t_total = ev[0].elapsed_time(ev[1]) * 1e-3
-    stage_ms = {name: float(np.mean([m[j].elapsed_time(m[j + 1]) for m in marks])) for j, (name, _) in enumerate(stages)}
+    t_total, stage_ms, per_step, next_offset = time_steps(torch, hp, args.steps, args.warmup, first_offset, stride, barrier)
     t_gen = stage_ms["generate"] * 1e-3
-    per_step = [m[0].elapsed_time(m[-1]) for m in marks]      # median and best beside the mean
     step_stats = {"median": float(np.median(per_step)), "best": float(np.min(per_step)), "worst": float(np.max(per_step))}
     n_acc_local = int(hp.n_acc.item()) if wl.unweight else 0
     if world > 1:
@@ -344,7 +516,7 @@ def run_ours(args):
         t_total, t_gen = float(tt[0]), float(tt[1])
     counts = gather_counts(n_acc_local)
     offsets = output_offsets(counts)
-    launches_all = sum(gather_counts(hp.launches(offset) * args.steps))   # ranks > 0 replay the pre-run: one more launch
+    launches_all = sum(gather_counts(hp.launches() * args.steps))
 
     # ---- end to end through the public API with HOST buffers: every step copies its input (the grid table) from pinned
     # host memory and the host reads the step's result.  For a generator the result is the unweighted sample: the
@@ -354,6 +526,7 @@ def run_ours(args):
     h_edges = torch.from_numpy(wl.grid()).pin_memory() if wl.grid() is not None else None
     h2d_bytes = h_edges.numel() * 8 if h_edges is not None else 0
     d2h_counter = [0]
+    e2e_offset = [next_offset]
     if wl.unweight:
         # output capacity of the e2e buffers: next power of two above twice the count seen in the device-resident run
         cap_e2e = min(hp.cap, max(1024, 1 << (2 * max(n_acc_local, 1) - 1).bit_length()))
@@ -372,10 +545,11 @@ def run_ours(args):
             s, h = k % 2, hps[k % 2]
             if h_edges is not None:                        # this step's input, uploaded while the previous step runs
                 with torch.cuda.stream(up_stream):
-                    h.d_edges.copy_(h_edges, non_blocking=True)
+                    h.d_edges.copy_(h_edges, non_blocking=True)   # same table: the cached w_max stays valid
                     ev_grid[s].record(up_stream)
                 stream.wait_event(ev_grid[s])
-            h.step(offset)
+            h.step(e2e_offset[0])
+            e2e_offset[0] += stride
             ev_done[s].record(stream)
             with torch.cuda.stream(down_stream):           # whole contiguous buffers: plain async memcpys into pinned memory
                 down_stream.wait_event(ev_done[s])
@@ -413,16 +587,18 @@ def run_ours(args):
             for _ in range(steps):
                 if h_edges is not None:
                     hp.d_edges.copy_(h_edges, non_blocking=True)
-                hp.step(offset)
+                hp.step(e2e_offset[0])
+                e2e_offset[0] += stride
                 for d_t, h_t in d2h:
                     h_t.copy_(d_t, non_blocking=True)
                 d2h_counter[0] = sum(h_t.numel() * h_t.element_size() for _, h_t in d2h)
                 torch.cuda.current_stream().synchronize()  # the host consumes the step's result
         e2e_what = "grid table H2D from pinned memory + whole step + D2H of all momenta and weights, host waits every step"
 
-    e2e_run(2)
+    e2e_run(3)
     barrier()
     t0 = time.perf_counter()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     ev[0].record(stream)
     e2e_run(args.steps)
     ev[1].record(stream)
@@ -439,35 +615,68 @@ def run_ours(args):
         if world > 1:
             dist.destroy_process_group()
         return 0
+    if world > 1:
+        dist.destroy_process_group()                       # nothing below communicates
+    if wl.unweight:
+        del hps, hb
+    torch.cuda.empty_cache()
 
-    # ---- roofline of the dominant kernel (the fused generation kernel)
-    hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
+    # ---- roofline of the dominant kernel (the fused generation kernel) and of every other stage
+    import bench_probes
     sms = torch.cuda.get_device_properties(local).multi_processor_count
-    bytes_per_launch = N * wl.out_bytes_per_event + (h2d_bytes if h_edges is not None else 0)
-    inst_per_event = alg_fp64_per_event(wl)
-    fp64_peak = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6            # fp64-pipe instructions / s at max clock
-    fp64_probe = probe_fp64_rate(ms, torch)
-    fp64_probe3 = probe_fp64_rate(ms, torch, three_regs=True)
-    write_probe = probe_write_stream(ms, torch, hp, wl)
-    t_hbm = bytes_per_launch / (hbm_gbs * 1e9)
-    t_alu = N * inst_per_event / fp64_peak
-    if t_hbm >= t_alu:
-        roof = {"bound": "hbm", "achieved": bytes_per_launch / t_gen / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+    peaks = measure_peaks(torch, sms)
+    write_probe = bench_probes.write_stream_gbs(torch, hp.N, hp.spec.rows_p, hp.p, hp.ld)
+    d_inv = 3 * wl.n - 4
+    traffic = dict(NCU_TRAFFIC.get(wl.name, {})) if N == wl.N else {}
+    if args.traffic > 0:
+        traffic["generate"] = (args.traffic, "--traffic")
+    stage_roof = {k: stage_roofline(k, wl, N, v, peaks, n_acc_local, d_inv, traffic.get(k)) for k, v in stage_ms.items()}
+    g = stage_roof["generate"]
+    bytes_per_launch = N * alg_bytes_per_event(wl)
+    inst_per_launch = N * alg_fp64_per_event(wl)
+    if g["bound"] == "hbm":
+        roof = {"bound": "hbm", "achieved": bytes_per_launch / t_gen / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
     else:
-        roof = {"bound": "alu", "achieved": N * inst_per_event / t_gen / 1e9, "peak": fp64_peak / 1e9, "unit": "Ginst/s (fp64 pipe)"}
+        roof = {"bound": "alu", "achieved": inst_per_launch / t_gen / 1e9, "peak": peaks["fp64_ginst_measured"],
+                "unit": "Ginst/s (fp64 pipe)"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    traffic, traffic_src = (args.traffic, "--traffic") if args.traffic > 0 else NCU_TRAFFIC.get(wl.name, (None, None))
-    if N != wl.N:
-        traffic, traffic_src = None, None
-    roof.update(traffic=traffic, traffic_source=traffic_src, kernel="ms::gen_kernel<%d,%s,%s>" % (
-        wl.n, "exact" if wl.mapping == "rambo" else "fast", "massive" if wl.masses else "massless"),
-        kernel_ms=1e3 * t_gen, kernel_share_of_step=t_gen * args.steps / t_total, peak_source=peak_src,
-        alg_bytes_per_event=wl.out_bytes_per_event, alg_fp64_inst_per_event=inst_per_event,
-        hbm_time_ms=1e3 * t_hbm, alu_time_ms=1e3 * t_alu, frac_of_max_side=max(t_hbm, t_alu) / t_gen,
-        fp64_peak_ginst_nominal=fp64_peak / 1e9, fp64_ginst_probe_measured=fp64_probe / 1e9, fp64_ginst_probe_3reg_operands=fp64_probe3 / 1e9, write_stream_probe_gbs=write_probe,
-        kernel_events_per_s=N / t_gen)
+    roof.update(traffic=g["traffic"], traffic_source=g["traffic_source"], kernel=g["kernel"], kernel_ms=1e3 * t_gen,
+                kernel_share_of_step=t_gen * args.steps / t_total,
+                peak_source="HBM: %s; fp64: measured here (%s)" % (peaks["hbm_source"], peaks["fp64_probe"]),
+                alg_bytes_per_event=g["alg_bytes_per_event"], alg_fp64_inst_per_event=g["alg_fp64_inst_per_event"],
+                hbm_time_ms=g["hbm_time_ms"], alu_time_ms=g["alu_time_ms"],
+                fp64_peak_ginst_nominal=peaks["fp64_ginst_nominal"], fp64_ginst_probe_measured=peaks["fp64_ginst_measured"],
+                fp64_ginst_probe_measured_best=peaks["fp64_ginst_measured_best"],
+                fp64_ginst_probe_3reg_operands=peaks["fp64_ginst_3reg_operands"],
+                imad_wide_ginst_probe_measured=peaks["imad_wide_ginst_measured"], write_stream_probe_gbs=write_probe,
+                kernel_events_per_s=N / t_gen)
 
     cb = None if args.skip_cpu_baseline else time_oracle(wl, target_seconds=12.0)[0]
+
+    per_config = None
+    if world == 1 and not args.skip_per_config and args.events <= 0:
+        fail_main = int(hp.fail.item())
+        per_config = {}
+        # the headline workload's own block: the stage rooflines above + parity on the buffers just used
+        head = {"workload": "%s: %s" % (wl.name, wl.note), "events_per_step": N, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": 1e3 * t_total / args.steps, "events_per_s": N * args.steps / t_total, "stages": stage_roof,
+                "kernel": g["kernel"], "kernel_ms": g["ms"], "bound": g["bound"], "frac": g["frac"],
+                "hbm_time_ms": g["hbm_time_ms"], "alu_time_ms": g["alu_time_ms"],
+                "alg_bytes_per_event": g["alg_bytes_per_event"], "alg_fp64_inst_per_event": g["alg_fp64_inst_per_event"],
+                "traffic": g["traffic"], "parity": parity_and_pins(torch, ms, hp, wl, wl.name), "cpu_baseline": cb}
+        if wl.unweight:
+            head["unweighted_events_per_s"] = sum(counts) * args.steps / t_total
+        per_config[wl.name] = head
+        del hp
+        torch.cuda.empty_cache()
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg4rw", "cfg5"):
+            if name == wl.name:
+                continue
+            per_config[name] = measure_config(torch, ms, name, args.per_config_steps, max(args.warmup, 3), peaks,
+                                              0.0 if args.skip_cpu_baseline else 4.0)
+    else:
+        fail_main = int(hp.fail.item())
+
     total_events = float(N) * world * args.steps
     line = {"metric": METRIC, "value": total_events / t_total, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -476,58 +685,13 @@ def run_ours(args):
             "e2e": {"value": total_events / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_counter[0],
                     "wall_value": total_events / t_e2e_wall,
                     "what": e2e_what},
-            "gpu_launches": launches_all, "roofline": roof, "stage_ms": stage_ms, "ms_per_step_stats": step_stats, "cpu_baseline": cb,
+            "gpu_launches": launches_all, "roofline": roof, "stage_ms": stage_ms, "stage_roofline": stage_roof,
+            "ms_per_step_stats": step_stats, "cpu_baseline": cb,
             "unweighted": ({"accepted_per_step_per_rank": counts, "global_offsets": offsets,
                             "unweighted_events_per_s": sum(counts) * args.steps / t_total} if wl.unweight else None),
-            "fail_count": int(hp.fail.item()),
+            "fail_count": fail_main, "per_config": per_config,
             "paper_context": "PAPER.md:766-770: full LO chain incl. matrix elements ~30M weighted evt/s on A100 (DY+1g), up to 10M on 24 Xeon-4214 cores; not this path in isolation"}
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
-    return 0
-
-
-def run_unweight_density(args):
-    """Side measurement (not the bench line): ms_unweight alone on 2^24 synthetic weights x 24 momentum rows at several
-    acceptance rates -- the unweighting efficiencies a production run sees after grid adaptation
-    rather than the 1e-4 of the seeded-grid workloads.  Weights w = u^(1/f - 1) with w_max = 1 have <w>/w_max = f."""
-    import torch
-    import paper_2602_06895_b200 as ms
-    ms.lib()
-    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
-    torch.cuda.set_device(dev)
-    N, rows = 1 << 24, 24
-    f64 = dict(dtype=torch.float64, device=dev)
-    gen = torch.Generator(device=dev)
-    gen.manual_seed(5)
-    p = torch.rand((rows, N), generator=gen, **f64)
-    idx = torch.empty(N, dtype=torch.int64, device=dev)
-    w_out, rows_out = torch.empty(N, **f64), torch.empty((rows, N), **f64)
-    n_acc = torch.zeros(1, dtype=torch.int64, device=dev)
-    sb = ms.ms_unweight_scratch_bytes(N)
-    scratch = torch.empty(sb, dtype=torch.uint8, device=dev)
-    wmax = torch.ones(1, **f64)
-    out = []
-    for frac in (1e-4, 1e-3, 1e-2, 0.1, 0.5, 1.0):
-        w = torch.rand(N, generator=gen, **f64) ** (1.0 / frac - 1.0)
-
-        def call():
-            ms.ms_unweight(N, w, wmax, ms.rng(ms_inputs.SEED_UNWEIGHT, 1, 0), rows, p, N, idx, w_out, rows_out, n_acc, scratch,
-                           sb, N, None)
-        for _ in range(max(args.warmup, 3)):
-            call()
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-        torch.cuda.synchronize()
-        ev[0].record()
-        for _ in range(args.steps):
-            call()
-        ev[1].record()
-        torch.cuda.synchronize()
-        us = ev[0].elapsed_time(ev[1]) * 1e3 / args.steps
-        k = int(n_acc.item())
-        moved = 8 * N + k * 16 * (rows + 2)                    # weights read + (idx, w_out, rows) read and written
-        out.append({"efficiency": frac, "accepted": k, "us_per_call": us, "algorithmic_gb_per_s": moved / us / 1e3})
-    print(json.dumps({"probe": "unweight-density", "events": N, "rows": rows, "steps": args.steps, "results": out}))
     return 0
 
 
@@ -540,13 +704,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=0, help="override events per GPU per step (0 = the workload's)")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: do not time the oracle")
+    ap.add_argument("--skip-per-config", action="store_true", help="profiling runs only: the headline workload alone")
+    ap.add_argument("--per-config-steps", type=int, default=10, help="timed steps of each non-headline config")
     ap.add_argument("--traffic", type=float, default=0.0, help="dram bytes per launch of the dominant kernel from ncu (recorded, not measured here)")
-    ap.add_argument("--probe", default="", choices=["", "unweight-density"],
-                    help="side measurements for DESIGN.md / profiles (not the bench line)")
     args = ap.parse_args()
-    if args.probe == "unweight-density":
-        args.steps = min(args.steps, 20)
-        return run_unweight_density(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 

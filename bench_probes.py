@@ -1,0 +1,260 @@
+#!/usr/bin/env python
+"""bench_probes.py -- measurement helpers used by bench.py and by the recipes under profiles/ (NOT part of the product
+library: the kernels live in bench_probes.cu and build into libms_bench_probes.so beside this file).
+
+    python bench_probes.py fp64              # sustained DFMA rate, >= 2 s per form, median and best
+    python bench_probes.py issue-model       # 4 DFMA + K other instructions per loop: which pipes issue beside the fp64 pipe
+    python bench_probes.py unweight-density  # ms_unweight alone at acceptance rates 1e-4 .. 1
+    python bench_probes.py chili             # ms_chili n = 3, 4, 6 at 2^24 events (CUDA events; ncu-able)
+
+Each prints one JSON line.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import json
+import os
+import shutil
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(ROOT, "bench_probes.cu")
+LIB = os.path.join(ROOT, "libms_bench_probes.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+        return LIB
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    tmp = LIB + ".tmp.%d" % os.getpid()
+    cmd = [nvcc, "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
+           "-shared", SRC, "-o", tmp]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    os.replace(tmp, LIB)
+    return LIB
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        vp, i64, i = C.c_void_p, C.c_int64, C.c_int
+        L.probe_dfma.argtypes = [i, i, vp, vp]
+        L.probe_dfma3.argtypes = [i, i, vp, vp]
+        L.probe_write.argtypes = [i64, i, vp, i64, vp]
+        L.probe_mix.argtypes = [i, i, i, i, i, vp, vp]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise RuntimeError("%s: cudaError %d" % (what, rc))
+
+
+def fp64_rate(torch, seconds: float = 2.0, three_regs: bool = False) -> dict:
+    """DFMA instructions/s sustained for `seconds` ("dependent-free DFMA loop sustained for
+    seconds"): back-to-back launches of 8 independent chains per thread, one CUDA-event pair per launch; the MEDIAN
+    launch is the figure the rooflines use, the best one is reported beside it."""
+    import numpy as np
+    fn = lib().probe_dfma3 if three_regs else lib().probe_dfma
+    s = torch.cuda.current_stream().cuda_stream
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    blocks, iters = sms * 8, 1 << 14
+    sink = torch.empty(blocks * 256, dtype=torch.float64, device="cuda")
+    inst = blocks * 256 * iters * 8
+    _check(fn(blocks, iters, sink.data_ptr(), s), "probe_dfma")
+    torch.cuda.synchronize()
+    rates, t_end = [], time.perf_counter() + seconds
+    while time.perf_counter() < t_end or len(rates) < 5:
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(9)]
+        evs[0].record()
+        for k in range(8):                               # 8 launches in flight: no host gap between them
+            _check(fn(blocks, iters, sink.data_ptr(), s), "probe_dfma")
+            evs[k + 1].record()
+        evs[-1].synchronize()
+        rates += [inst / (evs[k].elapsed_time(evs[k + 1]) * 1e-3) for k in range(8)]
+    return {"median": float(np.median(rates)), "best": float(np.max(rates)), "launches": len(rates),
+            "seconds": seconds, "form": "a*b+c, three registers" if three_regs else "a*const+const"}
+
+
+def write_stream_gbs(torch, N: int, rows: int, out, ld: int, reps: int = 10) -> float:
+    """GB/s of the generation kernel's store pattern with no arithmetic (rows x N doubles, streaming stores)."""
+    s = torch.cuda.current_stream().cuda_stream
+    _check(lib().probe_write(N, rows, out.data_ptr(), ld, s), "probe_write")
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(reps):
+        _check(lib().probe_write(N, rows, out.data_ptr(), ld, s), "probe_write")
+    ev1.record()
+    ev1.synchronize()
+    return 8.0 * rows * N * reps / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
+
+
+def imad_wide_rate(torch, reps: int = 5) -> float:
+    """32x32 -> 64-bit multiply-adds (IMAD.WIDE.U32, the multiply of a Philox round) per second, thread-level like the
+    DFMA figure: 8 independent chains per thread, all SMs busy with 8 warps per scheduler."""
+    s = torch.cuda.current_stream().cuda_stream
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    blocks, iters = sms * 4, 1 << 13
+    sink = torch.empty(blocks * 256, dtype=torch.float64, device="cuda")
+    _check(lib().probe_mix(3, 8, 0, blocks, iters, sink.data_ptr(), s), "probe_mix")
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(reps):
+        _check(lib().probe_mix(3, 8, 0, blocks, iters, sink.data_ptr(), s), "probe_mix")
+    ev1.record()
+    ev1.synchronize()
+    return blocks * 256 * iters * 8 * reps / (ev0.elapsed_time(ev1) * 1e-3)
+
+
+MIX_KINDS = {1: "LOP3", 2: "IMAD", 3: "IMAD.WIDE.U32", 4: "FFMA", 5: "MUFU.RCP (fp32)", 6: "F2I.F64 + I2F.F64 (pair)",
+             7: "LDS.64", 8: "IADD3", 9: "MUFU.RCP64H"}
+
+
+def issue_model(torch) -> dict:
+    """Cycles per loop iteration and warp scheduler (4 per SM) of [nd DFMA + k x kind], all SMs busy with 8 warps per
+    scheduler, at the SM clock nvidia-smi reports under this load."""
+    s = torch.cuda.current_stream().cuda_stream
+    props = torch.cuda.get_device_properties(torch.cuda.current_device())
+    sms = props.multi_processor_count
+    blocks, iters = sms * 4, 1 << 13                      # 4 blocks x 8 warps per SM = 8 warps per scheduler
+    sink = torch.empty(blocks * 256, dtype=torch.float64, device="cuda")
+
+    def cycles(kind, k, nd):
+        _check(lib().probe_mix(kind, k, nd, blocks, iters, sink.data_ptr(), s), "probe_mix")
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(5):
+            _check(lib().probe_mix(kind, k, nd, blocks, iters, sink.data_ptr(), s), "probe_mix")
+        ev1.record()
+        ev1.synchronize()
+        t = ev0.elapsed_time(ev1) * 1e-3 / 5
+        warp_iters_per_sched = blocks * 8 * iters / (sms * 4)
+        return t * clock_hz / warp_iters_per_sched
+
+    try:
+        q = subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"],
+                           capture_output=True, text=True).stdout.strip().splitlines()[0]
+        clock_hz = float(q) * 1e6
+    except Exception:
+        clock_hz = 1965e6
+    out = {"clock_mhz_assumed": clock_hz / 1e6, "unit": "cycles per iteration per scheduler (includes ~2-3 loop instructions)",
+           "dfma4_alone": cycles(0, 0, 4), "rows": []}
+    for kind, name in MIX_KINDS.items():
+        out["rows"].append({"kind": name, "k4_alone": cycles(kind, 4, 0), "k8_alone": cycles(kind, 8, 0),
+                            "dfma4_plus_k2": cycles(kind, 2, 4), "dfma4_plus_k4": cycles(kind, 4, 4),
+                            "dfma4_plus_k8": cycles(kind, 8, 4)})
+    return out
+
+
+def unweight_density(torch, steps: int = 20, warmup: int = 3) -> dict:
+    """ms_unweight alone on 2^24 synthetic weights x 24 momentum rows at several acceptance rates -- the unweighting
+    efficiencies a production run sees after grid adaptation rather than the 1e-4 of the seeded-grid
+    workloads.  Weights w = u^(1/f - 1) with w_max = 1 have <w>/w_max = f."""
+    sys.path.insert(0, ROOT)
+    import ms_inputs
+    import paper_2602_06895_b200 as ms
+    ms.lib()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    N, rows = 1 << 24, 24
+    f64 = dict(dtype=torch.float64, device=dev)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(5)
+    p = torch.rand((rows, N), generator=gen, **f64)
+    idx = torch.empty(N, dtype=torch.int64, device=dev)
+    w_out, rows_out = torch.empty(N, **f64), torch.empty((rows, N), **f64)
+    n_acc = torch.zeros(1, dtype=torch.int64, device=dev)
+    sb = ms.ms_unweight_scratch_bytes(N)
+    scratch = torch.empty(sb, dtype=torch.uint8, device=dev)
+    wmax = torch.ones(1, **f64)
+    out = []
+    for frac in (1e-4, 1e-3, 1e-2, 0.1, 0.5, 1.0):
+        w = torch.rand(N, generator=gen, **f64) ** (1.0 / frac - 1.0)
+
+        def call():
+            ms.ms_unweight(N, w, wmax, ms.rng(ms_inputs.SEED_UNWEIGHT, 1, 0), rows, p, N, idx, w_out, rows_out, n_acc, scratch,
+                           sb, N, None)
+        for _ in range(max(warmup, 3)):
+            call()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(steps):
+            call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        us = ev[0].elapsed_time(ev[1]) * 1e3 / steps
+        k = int(n_acc.item())
+        moved = 8 * N + k * 16 * (rows + 2)                    # weights read + (idx, w_out, rows) read and written
+        out.append({"efficiency": frac, "accepted": k, "us_per_call": us, "algorithmic_gb_per_s": moved / us / 1e3})
+    return {"probe": "unweight-density", "events": N, "rows": rows, "steps": steps, "results": out}
+
+
+def chili(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) -> dict:
+    """ms_chili at 2^24 events, Philox in-kernel, pT_min = 20 GeV on every particle, sqrt(s) = 13 TeV."""
+    sys.path.insert(0, ROOT)
+    import paper_2602_06895_b200 as ms
+    ms.lib()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    N = 1 << 24
+    out = []
+    for n in (3, 4, 6):
+        p = torch.empty((4 * (n + 2), N), dtype=torch.float64, device=dev)
+        w = torch.empty(N, dtype=torch.float64, device=dev)
+
+        def call():
+            ms.ms_chili(N, n, 13000.0 ** 2, None, [20.0] * n, None, None, ms.rng(1, 0, 0), p, w, None, N)
+        for _ in range(warmup):
+            call()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(steps):
+            call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        ms_call = ev[0].elapsed_time(ev[1]) / steps
+        nbytes = 8 * (4 * (n + 2) + 1) * N
+        row = {"n": n, "ms": ms_call, "alg_bytes": nbytes, "achieved_gbs": nbytes / ms_call / 1e6}
+        if hbm_gbs > 0:
+            row["frac_of_hbm"] = row["achieved_gbs"] / hbm_gbs
+        out.append(row)
+        del p, w
+    return {"probe": "chili", "events": N, "steps": steps, "results": out}
+
+
+def main() -> int:
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_probes.py needs a CUDA device")
+    what = sys.argv[1] if len(sys.argv) > 1 else "fp64"
+    if what == "fp64":
+        res = {"probe": "fp64", "const_operand": fp64_rate(torch, 2.0), "three_registers": fp64_rate(torch, 2.0, True)}
+    elif what == "issue-model":
+        res = {"probe": "issue-model", **issue_model(torch)}
+    elif what == "unweight-density":
+        res = unweight_density(torch)
+    elif what == "chili":
+        hbm = 0.0
+        pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(pk):
+            with open(pk) as f:
+                hbm = float(json.load(f)["hbm_gbs"])
+        res = chili(torch, hbm_gbs=hbm)
+    else:
+        raise SystemExit("unknown probe: " + what)
+    print(json.dumps(res))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

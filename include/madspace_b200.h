@@ -22,6 +22,7 @@
  *    uniform j takes output words (0,1) if j is even, (2,3) if odd: W = w_a<<32 | w_b,
  *    u = (2*(W>>12)+1) * 2^-53, in the open interval (0,1) (readings R-1..R-3).
  *    Wherever a uniform-row pointer may be NULL, NULL means "draw the uniforms in-kernel".
+ *  - N <= MS_MAX_EVENTS = 2^31 events per call of the phase-space entry points (MS_EINVAL beyond).
  *  - Return value: MS_OK, or a negative code detected on the host BEFORE any launch (nothing was
  *    enqueued), or MS_ECUDA when a launch failed (raw cudaError_t: ms_last_cuda_error()).
  *  - Per-event failures (Newton cap hit, non-finite weight) do not fail the call: the event gets
@@ -40,6 +41,9 @@ extern "C" {
 
 #define MS_MAX_N 9
 #define MS_MAX_DIMS 32      /* VEGAS grid dimensions */
+#define MS_MAX_EVENTS ((int64_t)1 << 31) /* events per call of the per-multiplicity kernels (ms_generate, ms_fastrambo,
+                                            ms_rambo_*, ms_fastrambo_inverse, ms_chili): 32-bit local event index;
+                                            longer batches are split by the caller (advance rng.event_offset) */
 #define MS_MAX_BINS 1024    /* VEGAS bins per dimension; d*(n_bins+1)*16 B must fit 200 KB of shared memory */
 
 enum {
@@ -116,7 +120,10 @@ int ms_fastrambo(int64_t N, int n, double sqrt_s, const double* d_sqrt_s, const 
 
 /* ms_fastrambo_inverse -- analytic inverse of ms_fastrambo (Eq. 64; readings F-1..F-5).
  * Reads the outgoing rows 8.. of d_p (any frame in which they were generated from Q_1 = sum p),
- * writes d_x [3n-4][ld] and, if d_w != NULL, the same weight the forward map returns. */
+ * writes d_x [3n-4][ld] and, if d_w != NULL, the same weight the forward map returns.
+ * Degenerate input (no inverse exists): a subsystem Q_i with Q_i^2 <= 0 after rounding (an exactly collinear massless
+ * pair) is given the mass 2^-500 Q_i^0, so every output stays finite and inside [0,1] (its mass uniform is 0, its
+ * angles arbitrary), and the event's d_w is 0; a particle with zero momentum gets cos theta uniform 1/2, azimuth 0. */
 int ms_fastrambo_inverse(int64_t N, int n, const double* d_p, double* d_x, double* d_w, int64_t ld, void* stream);
 
 /* ms_massive_rescale -- massive extension, strategy (i) of PAPER.md:510 (momentum rescaling of classic
@@ -184,7 +191,9 @@ int ms_reduce_max(int64_t N, const double* d_w, double* d_out, void* stream);
  *   accepted events are written in increasing event order: d_idx[k] = e, d_w_out[k] = max(1, w_e/w_max),
  *   d_rows_out[r*cap + k] = d_rows_in[r*ld + e] for r < n_rows (skipped if either pointer is NULL).
  *   *d_n_accepted = true number accepted; only the first `cap` are stored.
- * d_wmax: device scalar.  d_scratch: ms_unweight_scratch_bytes(N) bytes (68 B per 512 events + 64 KB), any content, 16-byte
+ * d_wmax: device scalar; precondition 0 < w_max < inf.  If it is violated (every pre-run weight 0 under tight cuts, a
+ * non-finite maximum) NOTHING is accepted: *d_n_accepted = 0 and no output is written -- the caller sees an empty sample
+ * instead of infinite output weights.  d_scratch: ms_unweight_scratch_bytes(N) bytes (68 B per 512 events + 64 KB), any content, 16-byte
  * aligned; overwritten. */
 size_t ms_unweight_scratch_bytes(int64_t N);
 int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, int n_rows, const double* d_rows_in,
@@ -271,17 +280,6 @@ int ms_generate(const ms_gen_config* cfg, int64_t N, ms_rng rng, const double* d
 
 /* ms_fill_uniforms -- materialise Philox uniforms j = 0..d-1 as rows d_r[d][ld] (step S0 on its own). */
 int ms_fill_uniforms(int64_t N, int d, ms_rng rng, double* d_r, int64_t ld, void* stream);
-
-/* ms_probe_dfma -- measurement helper: `iters` dependent-free DFMA chains per thread on `blocks` x 256
- * threads; d_sink receives one double per thread.  Executes blocks*256*iters*8 DFMA. */
-int ms_probe_dfma(int blocks, int iters, double* d_sink, void* stream);
-
-/* ms_probe_dfma3 -- as ms_probe_dfma, but every DFMA has three distinct register operands (a*b+c). */
-int ms_probe_dfma3(int blocks, int iters, double* d_sink, void* stream);
-
-/* ms_probe_write -- measurement helper: the generation kernel's store pattern with no arithmetic: every event
- * writes `rows` doubles, one per SoA row of d_out[rows][ld], with streaming stores (8*rows*N bytes per call). */
-int ms_probe_write(int64_t N, int rows, double* d_out, int64_t ld, void* stream);
 
 #ifdef __cplusplus
 }

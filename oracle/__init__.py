@@ -16,7 +16,10 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libms_oracle.so")
+# MS_ORACLE_SANITIZE=1 (tests/test_oracle_sanitizers.py, in a subprocess with libasan preloaded): the same sources built
+# with -fsanitize=address,undefined into a second library; the arithmetic flags are unchanged.
+_SANITIZE = os.environ.get("MS_ORACLE_SANITIZE", "") == "1"
+_SO = os.path.join(_HERE, "libms_oracle_san.so" if _SANITIZE else "libms_oracle.so")
 _SRCS = [os.path.join(_HERE, "ms_oracle.c"), os.path.join(_HERE, "ms_oracle_lit.c")]
 
 
@@ -26,8 +29,10 @@ def build(force: bool = False) -> str:
     if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in srcs):
         return _SO
     tmp = _SO + ".tmp.%d" % os.getpid()
-    cmd = ["gcc", "-std=gnu11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-o", tmp] + srcs + ["-lquadmath", "-lm"]
+    opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=all"] if _SANITIZE \
+        else ["-O2"]
+    cmd = ["gcc", "-std=gnu11"] + opt + ["-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
+                                         "-Wall", "-o", tmp] + srcs + ["-lquadmath", "-lm"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, _SO)
     return _SO

@@ -24,7 +24,7 @@ _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECU
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_fill_uniforms", "ms_probe_dfma", "ms_probe_dfma3", "ms_probe_write")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_fill_uniforms")
 
 
 class MadSpaceError(RuntimeError):
@@ -87,9 +87,6 @@ def lib() -> C.CDLL:
         L.ms_reduce_max.argtypes = [_i64, _vp, _vp, _vp]
         L.ms_unweight.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
         L.ms_generate.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp]
-        L.ms_probe_dfma.argtypes = [_int, _int, _vp, _vp]
-        L.ms_probe_dfma3.argtypes = [_int, _int, _vp, _vp]
-        L.ms_probe_write.argtypes = [_i64, _int, _vp, _i64, _vp]
         _lib = L
     return _lib
 
@@ -213,18 +210,6 @@ def gen_config(n, mapping="fastrambo", sqrt_s=0.0, grid_dims=0, grid_bins=0, pdf
 def ms_generate(cfg: ms_gen_config, N, r: ms_rng, d_edges, d_p, d_w, d_x1x2, ld, d_fail=None, stream=None) -> None:
     _check("ms_generate", lib().ms_generate(C.byref(cfg), N, r, _ptr(d_edges), _ptr(d_p), _ptr(d_w), _ptr(d_x1x2), ld,
                                             _ptr(d_fail), _stream(stream)))
-
-
-def ms_probe_dfma(blocks, iters, d_sink, stream=None) -> None:
-    _check("ms_probe_dfma", lib().ms_probe_dfma(blocks, iters, _ptr(d_sink), _stream(stream)))
-
-
-def ms_probe_write(N, rows, d_out, ld, stream=None) -> None:
-    _check("ms_probe_write", lib().ms_probe_write(N, rows, _ptr(d_out), ld, _stream(stream)))
-
-
-def ms_probe_dfma3(blocks, iters, d_sink, stream=None) -> None:
-    _check("ms_probe_dfma3", lib().ms_probe_dfma3(blocks, iters, _ptr(d_sink), _stream(stream)))
 
 
 def ms_rambo_massive_reweight(N, n, mapping, sqrt_s, masses: Sequence[float], d_x, r: ms_rng, d_p, d_w, ld,

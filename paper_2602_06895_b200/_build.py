@@ -49,6 +49,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
         return LIB
     os.makedirs(BUILD, exist_ok=True)
+    # one builder at a time: under torchrun every rank calls lib() -> build(), and all of them would compile into the
+    # same csrc/build/*.o paths; the others wait here and then find the library up to date
+    import fcntl
+    with open(os.path.join(BUILD, ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
+                return LIB
+            return _build_locked(verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose: bool) -> str:
     jobs = [(os.path.join(CSRC, "ms_api.cu"), os.path.join(BUILD, "ms_api.o"), ["-I", INCLUDE])]
     for n in N_RANGE:                                  # largest multiplicities first: they take longest
         for part in (0, 1, 2):

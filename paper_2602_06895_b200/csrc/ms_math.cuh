@@ -197,7 +197,7 @@ __device__ __forceinline__ double atan2_turns(double y, double x)
     const bool big = mn > 0x1.a827999fcef32p-2 * mx;            // tan(pi/8)
     const double num = big ? mn - mx : mn;
     const double den = big ? mn + mx : mx;
-    const double t = num * rcp_fast(den);
+    const double t = num * rcp_fast(fmax(den, 0x1p-1000));      // x = y = 0 (no azimuth): turn 0, not NaN
     double turn = fma(t, horner<12>(c_PA, t * t), big ? 0.125 : 0.0);
     if (swap) turn = 0.25 - turn;
     if (x < 0.0) turn = 0.5 - turn;

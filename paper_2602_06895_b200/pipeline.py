@@ -2,7 +2,7 @@
 tests check).  Marshalling and buffer ownership only: every arithmetic step is a call into the C ABI.
 
 One step = ms_generate (Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [rescale] -> [boost] -> [toy] -> weight)
-           [-> ms_reduce_max over the pre-run events -> ms_unweight (accept + stable compaction)]
+           [-> ms_unweight (accept + stable compaction) against w_max of the pre-run, computed once per grid]
            [-> ms_fastrambo_inverse -> ms_vegas_map(inverse)]            (round trip, cfg 5)
 """
 from __future__ import annotations
@@ -93,6 +93,7 @@ class HotPath:
             self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
             self._pre = None                                   # buffers of the replayed pre-run, allocated on first use
             self.fail_pre = torch.zeros(1, dtype=torch.int32, device=self.device)
+            self._wmax_cached = False                          # w_max is a function of (spec, grid): computed once
         if spec.inverse:
             self.d_inv = 3 * spec.n - 4
             self.x_inv = torch.empty((self.d_inv, self.ld), **f64)
@@ -104,6 +105,7 @@ class HotPath:
         if ms_check_grid(h_edges) != 0:
             raise MadSpaceError("ms_check_grid", MS_EGRID)
         self.grid_dims, self.grid_bins = h_edges.shape[0], h_edges.shape[1] - 1
+        self._wmax_cached = False                              # a new grid changes every weight, hence w_max
         # unused trailing dimensions whose bins all have n_bins * width == 1.0 exactly contribute a Jacobian of exactly 1
         tail = h_edges[self.spec.d_used:]
         self.tail_unit_jacobian = bool(tail.shape[0] > 0 and np.all(self.grid_bins * np.diff(tail, axis=1) == 1.0))
@@ -133,25 +135,37 @@ class HotPath:
             self.set_grid(new_edges)
         return new_edges
 
-    def unweight(self, event_offset: int = 0, stream=None, _wmax_zeroed: bool = False) -> None:
+    def invalidate_wmax(self) -> None:
+        """Forget the cached w_max (set_grid does it; call it after changing anything else the weights depend on)."""
+        self._wmax_cached = False
+
+    def ensure_wmax(self, stream=None) -> None:
+        """w_max = the maximum weight of the pre-run, the GLOBAL events 0..prerun-1 of the event stream (reading R-4;
+        BASELINE.json cfg 2: "w_max = max weight of a 2^16-event pre-run"), whatever range a batch or a rank owns.  It is
+        a pure function of (spec, grid), so it is computed ONCE per grid -- a deterministic replay of those events into a
+        13 MB side buffer, no communication between ranks -- and kept on the device until
+        set_grid() / invalidate_wmax(); fail_pre counts the pre-run's failed events."""
+        if self._wmax_cached:
+            return
         s = self.spec
         with _on(stream):
-            if not _wmax_zeroed:
-                self.wmax.zero_()
-            if event_offset == 0 and self.N >= s.prerun:
-                ms_reduce_max(s.prerun, self.w, self.wmax, None)    # the batch starts with the pre-run events
-            else:
-                # w_max is the maximum over the GLOBAL events 0..prerun-1 (reading R-4), whatever range this batch or
-                # this rank owns: replay them (deterministic, no communication)
-                if self._pre is None:
-                    ld = (s.prerun + 1) // 2 * 2
-                    f64 = dict(dtype=torch.float64, device=self.device)
-                    self._pre = (torch.empty((s.rows_p, ld), **f64), torch.empty(ld, **f64),
-                                 torch.empty((2, ld), **f64) if s.pdf else None, ld)
-                p_pre, w_pre, x_pre, ld = self._pre
-                ms_generate(self.cfg, s.prerun, rng(s.seed_events, 0, 0), self.d_edges, p_pre, w_pre, x_pre, ld,
-                            self.fail_pre, None)
-                ms_reduce_max(s.prerun, w_pre, self.wmax, None)
+            if self._pre is None:
+                ld = (s.prerun + 1) // 2 * 2
+                f64 = dict(dtype=torch.float64, device=self.device)
+                self._pre = (torch.empty((s.rows_p, ld), **f64), torch.empty(ld, **f64),
+                             torch.empty((2, ld), **f64) if s.pdf else None, ld)
+            p_pre, w_pre, x_pre, ld = self._pre
+            self.wmax.zero_()
+            self.fail_pre.zero_()
+            ms_generate(self.cfg, s.prerun, rng(s.seed_events, 0, 0), self.d_edges, p_pre, w_pre, x_pre, ld,
+                        self.fail_pre, None)
+            ms_reduce_max(s.prerun, w_pre, self.wmax, None)
+        self._wmax_cached = True
+
+    def unweight(self, event_offset: int = 0, stream=None) -> None:
+        s = self.spec
+        self.ensure_wmax(stream)
+        with _on(stream):
             ms_unweight(self.N, self.w, self.wmax, rng(s.seed_unweight, 1, event_offset), s.rows_p if self.gather_rows else 0,
                         self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
                         self.scratch, self.scratch_bytes, self.ld, None)
@@ -173,15 +187,23 @@ class HotPath:
 
     def step(self, event_offset: int = 0, stream=None) -> None:
         if self.spec.unweight:
-            # w_max is zeroed BEFORE the generation kernel, so that ms_reduce_max follows it directly in the stream and
-            # its programmatic dependent launch overlaps the generation kernel's tail
-            with _on(stream):
-                self.wmax.zero_()
+            self.ensure_wmax(stream)
         self.generate(event_offset, stream)
         if self.spec.unweight:
-            self.unweight(event_offset, stream, _wmax_zeroed=True)
+            self.unweight(event_offset, stream)
         if self.spec.inverse:
             self.invert(stream)
+
+    def stages(self):
+        """(name, callable(event_offset)) of one step, in order: what bench.py brackets with CUDA events."""
+        out = [("generate", lambda off: self.generate(off))]
+        if self.spec.unweight:
+            out.append(("unweight", lambda off: self.unweight(off)))
+        if self.spec.inverse:
+            out.append(("fastrambo_inverse", lambda off: self.invert_phase_space()))
+            if self.d_edges is not None:
+                out.append(("vegas_inverse", lambda off: self.invert_grid()))
+        return out
 
     def capture(self, event_offset: int = 0) -> "torch.cuda.CUDAGraph":
         """One step recorded as a CUDA graph (the library calls neither allocate nor synchronise, so a step is
@@ -199,12 +221,10 @@ class HotPath:
         return g
 
     def launches(self, event_offset: int = 0) -> int:
-        """Kernels of this library enqueued by one step(event_offset) (memsets/copies not counted)."""
+        """Kernels of this library enqueued by one step in steady state (w_max cached; memsets/copies not counted)."""
         k = 1
         if self.spec.unweight:
-            k += 3                                  # ms_reduce_max + decide / scatter of ms_unweight
-            if not (event_offset == 0 and self.N >= self.spec.prerun):
-                k += 1                              # the replayed pre-run (ms_generate over events 0..prerun-1)
+            k += 2                                  # decide / scatter of ms_unweight
         if self.spec.inverse:
             k += 2 if self.d_edges is not None else 1
         return k

@@ -95,6 +95,21 @@ def test_host_side_argument_errors(ms):
     assert _code(ms, ms.ms_fastrambo, 8, 4, 1000.0, None, None, bad, FAKE, FAKE, 8, None, 0) == ms.MS_EINVAL
 
 
+def test_batches_beyond_the_32_bit_event_index_are_rejected(ms):
+    """The per-multiplicity kernels index events with 32 bits; N > MS_MAX_EVENTS = 2^31 returns MS_EINVAL before any
+    launch instead of silently processing N mod 2^32 events."""
+    r0, big = ms.rng(1), (1 << 31) + 1
+    assert _code(ms, ms.ms_fastrambo, big, 4, 1000.0, None, None, r0, FAKE, FAKE, big + 1, None, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_rambo_massless, 1 << 32, 4, 1000.0, None, None, r0, FAKE, FAKE, 1 << 32, None, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_rambo_massive_reweight, big, 4, "fastrambo", 2000.0, (173.0, 173.0, 0.0, 0.0), None, r0, FAKE, FAKE,
+                 big + 1, None, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_fastrambo_inverse, big, 4, FAKE, FAKE, None, big + 1, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_rambo_massive_reweight_inverse, big, 4, (173.0, 173.0, 0.0, 0.0), FAKE, FAKE, None, big + 1, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_chili, big, 3, 1e8, None, None, None, None, r0, FAKE, FAKE, None, big + 1, 0) == ms.MS_EINVAL
+    cfg = ms.gen_config(4, "fastrambo", 1000.0)
+    assert _code(ms, ms.ms_generate, cfg, big, r0, None, FAKE, FAKE, None, big + 1, None, 0) == ms.MS_EINVAL
+
+
 def test_empty_batches_are_no_ops(ms):
     r0 = ms.rng(1)
     ms.ms_fastrambo(0, 4, 1000.0, None, None, r0, FAKE, FAKE, 0, None, 0)

@@ -48,6 +48,10 @@ def test_roofline_inputs_follow_the_workloads():
         wl = ms_inputs.WORKLOADS[name]
         assert wl.out_rows == rows and wl.out_bytes_per_event == 8 * rows
         assert bench.alg_fp64_per_event(wl) > 0
+        # the x1, x2 rows the kernel stores where Bjorken x are sampled count as algorithmic bytes
+        assert bench.alg_bytes_per_event(wl) == 8 * rows + (16 if wl.pdf else 0)
+    assert bench.alg_fp64_inverse(8) > bench.alg_fp64_inverse(4) > 0
+    assert set(bench.CLOSED_FORM) == set(ms_inputs.WORKLOADS)
     # the hand count grows with the multiplicity and with every optional stage
     c = {k: bench.alg_fp64_per_event(ms_inputs.WORKLOADS[k]) for k in ms_inputs.WORKLOADS}
     assert c["cfg1"] < c["cfg2"] < c["cfg5"] and c["cfg4rw"] < c["cfg4"]
@@ -68,7 +72,7 @@ def test_our_arm_prints_one_contract_line_on_the_gpu():
               "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
         assert k in d, k
     assert d["steps"] == 3 and d["warmup"] == 3 and d["n_gpus"] == 1 and d["scaling"] == "weak" and d["dtype"] == "f64"
-    assert d["gpu_launches"] == 4 * 3                      # generate, reduce_max, decide, scatter per step
+    assert d["gpu_launches"] == 3 * 3                      # per step in steady state: generate, decide, scatter
     r = d["roofline"]
     assert r["bound"] in ("hbm", "alu") and r["unit"].split()[0] in ("GB/s", "Ginst/s") and r["peak"] > 0
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0 < r["frac"] < 1.0
@@ -76,3 +80,43 @@ def test_our_arm_prints_one_contract_line_on_the_gpu():
     assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     assert d["fail_count"] == 0 and d["unweighted"]["accepted_per_step_per_rank"][0] > 0
     assert "sm_mhz" in d["clocks"] and "reasons" in d["clocks"]
+
+
+PER_CONFIG_KEYS = ("kernel", "kernel_ms", "alg_bytes_per_event", "alg_fp64_inst_per_event", "hbm_time_ms", "alu_time_ms", "bound",
+                   "frac", "traffic", "stages", "parity", "ms_per_step", "events_per_s")
+STAGE_KEYS = ("ms", "bound", "roofline_ms", "frac", "traffic", "kernel")
+
+
+@pytest.mark.gpu
+def test_per_config_block_covers_every_config_and_stage():
+    """one bench command measures all BASELINE.json configs -- every stage with its own roofline against
+    the MEASURED fp64 rate, sampled parity against the oracle, the round-trip exceedance count and the Monte Carlo mean
+    against the closed forms."""
+    out = run_bench("--steps", "3", "--warmup", "3", "--per-config-steps", "2", "--skip-cpu-baseline").strip().splitlines()
+    assert len(out) == 1
+    d = json.loads(out[0])
+    pc = d["per_config"]
+    assert set(pc) == {"cfg1", "cfg2", "cfg3", "cfg4", "cfg4rw", "cfg5"}
+    assert d["roofline"]["fp64_ginst_probe_measured"] > 0.5 * d["roofline"]["fp64_peak_ginst_nominal"]
+    for name, c in pc.items():
+        for k in PER_CONFIG_KEYS:
+            assert k in c, (name, k)
+        assert c["bound"] in ("hbm", "alu") and 0 < c["frac"] < 1.1
+        want = {"generate"} | ({"unweight"} if name in ("cfg2", "cfg5") else set()) \
+            | ({"fastrambo_inverse", "vegas_inverse"} if name == "cfg5" else set())
+        assert set(c["stages"]) == want, (name, set(c["stages"]))
+        for st in c["stages"].values():
+            for k in STAGE_KEYS:
+                assert k in st
+        par = c["parity"]
+        assert par["max_dp_over_sqrt_s"] <= 1e-12 and par["fail_count"] == 0
+        mc = par["mc_mean_over_closed_form"]
+        if name == "cfg5":      # d = 20 on a random grid: heavy-tailed, a weak pin (BASELINE.md section 2)
+            assert 0.5 < mc["ratio"] < 2.0, mc
+        else:
+            assert abs(mc["ratio"] - 1.0) <= 5.0 * mc["mc_error"] + 1e-13, (name, mc)
+    assert pc["cfg3"]["alg_bytes_per_event"] == 248
+    assert pc["cfg2"]["parity"]["unweighting_bit_exact_vs_oracle_on_all_weights"] is True
+    assert pc["cfg5"]["parity"]["unweighting_bit_exact_vs_oracle_on_all_weights"] is True
+    assert pc["cfg5"]["parity"]["round_trip"]["events_with_dr_above_1e-10"] <= 1024
+    assert "cuda_graph_replay_ms_per_step" in pc["cfg1"]

@@ -12,7 +12,7 @@ import pytest
 import torch
 
 import ms_inputs
-from helpers import oracle_chain, path_spec, toy_condition
+from helpers import assert_toy_weights, inverse_weight_bound, oracle_chain, path_spec
 
 pytestmark = pytest.mark.gpu
 
@@ -37,7 +37,7 @@ def sample_indices(N, seed):
     return np.unique(np.concatenate(parts)).astype(np.int64)
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg4rw", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg4rw", "cfg5"])
 def test_full_size_step(ms, orc, name):
     from paper_2602_06895_b200.pipeline import HotPath
     wl = ms_inputs.WORKLOADS[name]
@@ -57,11 +57,22 @@ def test_full_size_step(ms, orc, name):
     assert eta <= TOL_P, "max |dp|/E_scale = %.3e" % eta
     rel = np.abs(w - ref["w"]) / ref["w"]
     if wl.toy:
-        kappa = toy_condition(ref["p"], n, wl.sqrt_s)
-        assert np.all(rel <= TOL_W + 4.0 * max(eta, 2.3e-16) * kappa)
-        assert np.mean(rel <= TOL_W) > 0.999
+        assert_toy_weights(w, ref["w"], ref["p"], n, wl.sqrt_s, eta, "%s full size, %d sampled events" % (name, idx.size))
     else:
         assert np.max(rel) <= TOL_W, "max rel dw = %.3e" % np.max(rel)
+
+    # ---- cfg 1 (k = 1, c = 2 makes FastRambo exact): EVERY weight of the 2^16
+    # events equals Phi_3(1000 GeV) = 125.982556379686 GeV^2, and the step replayed from a CUDA graph (how a sub-wave
+    # batch is run without launch latency) reproduces the buffers bit for bit
+    if name == "cfg1":
+        assert float((hp.w[:N] / 125.982556379686 - 1.0).abs().max()) < 1e-13
+        p0, w0 = hp.p.clone(), hp.w.clone()
+        g = hp.capture(0)
+        hp.p.fill_(-7.0)
+        hp.w.fill_(-7.0)
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(hp.p, p0) and torch.equal(hp.w, w0)
 
     # ---- properties over ALL events, on the device
     assert bool(torch.isfinite(hp.w[:N]).all()) and bool((hp.w[:N] > 0).all())
@@ -133,4 +144,7 @@ def test_full_size_step(ms, orc, name):
         # the inverse returns the forward phase-space weight
         w_ps = hp.w_inv[t_idx].cpu().numpy()
         rel_ps = np.abs(w_ps - ref["w_ps"]) / ref["w_ps"]
-        assert np.median(rel_ps) <= 1e-13 and np.quantile(rel_ps, 0.99) <= 1e-10
+        bound = inverse_weight_bound(ref["p"], n)                        # reading F-8
+        print("inverse weight vs forward weight: max rel = %.3e, max rel/bound = %.3g, beyond 1e-12: %d of %d"
+              % (rel_ps.max(), (rel_ps / bound).max(), int((rel_ps > 1e-12).sum()), rel_ps.size))
+        assert np.all(rel_ps <= bound) and np.median(rel_ps) <= 1e-13
