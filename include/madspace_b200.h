@@ -44,6 +44,7 @@ extern "C" {
 #define MS_MAX_EVENTS ((int64_t)1 << 31) /* events per call of the per-multiplicity kernels (ms_generate, ms_fastrambo,
                                             ms_rambo_*, ms_fastrambo_inverse, ms_chili): 32-bit local event index;
                                             longer batches are split by the caller (advance rng.event_offset) */
+#define MS_MAX_LD ((int64_t)0xFFFFFFFF)     /* row stride of those calls: a 32-bit element count */
 #define MS_MAX_BINS 1024    /* VEGAS bins per dimension; d*(n_bins+1)*16 B must fit 200 KB of shared memory */
 
 enum {
@@ -83,7 +84,8 @@ int ms_check_grid(int d, int n_bins, const double* h_edges);
  *       The quotient is the IEEE-754 correctly rounded one (the divisor-only part of div.rn.f64 is tabulated per
  *       bin; inputs outside its fast path go through div.rn.f64 itself): results are bit-identical to a / b on the host.
  * d_edges: device table [d][n_bins+1], validated by the caller with ms_check_grid.
- * d_out: [d][ld].  d_jac: [N] or NULL.  d_in and d_out may alias.
+ * d_out: [d][ld].  d_jac: [N] or NULL.  d_in and d_out may be the same buffer (in place) or disjoint; a partial
+ * overlap is rejected (MS_EINVAL).
  * Errors: MS_EINVAL on bad sizes or pointers, or if the tables exceed 200 KB of shared memory
  * (forward: 16 d n_bins bytes; inverse: 16 d (n_bins+1) + 4 d 2^ceil(log2 n_bins) bytes). */
 int ms_vegas_map(int64_t N, int d, int n_bins, const double* d_edges, int direction,
@@ -122,13 +124,14 @@ int ms_fastrambo(int64_t N, int n, double sqrt_s, const double* d_sqrt_s, const 
  * Reads the outgoing rows 8.. of d_p (any frame in which they were generated from Q_1 = sum p),
  * writes d_x [3n-4][ld] and, if d_w != NULL, the same weight the forward map returns.
  * Degenerate input (no inverse exists): a subsystem Q_i with Q_i^2 <= 0 after rounding (an exactly collinear massless
- * pair) is given the mass 2^-500 Q_i^0, so every output stays finite and inside [0,1] (its mass uniform is 0, its
+ * pair) is given the mass 2^-500 Q_i^0, so every output stays finite and inside [0,1] (its mass uniform is below 1e-290, its
  * angles arbitrary), and the event's d_w is 0; a particle with zero momentum gets cos theta uniform 1/2, azimuth 0. */
 int ms_fastrambo_inverse(int64_t N, int n, const double* d_p, double* d_x, double* d_w, int64_t ld, void* stream);
 
 /* ms_massive_rescale -- massive extension, strategy (i) of PAPER.md:510 (momentum rescaling of classic
  * RAMBO, ref. [64]; readings K-1..K-3): solve sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt_s for xi by Newton
- * in registers until |F| <= rel_tol*sqrt_s (at most max_iter steps), k_i = (sqrt(m_i^2+xi^2 E_i^2), xi p_i),
+ * in registers (the first two steps are Halley's third-order variant of the Newton step, the rest plain Newton) until
+ * |F| <= rel_tol*sqrt_s (at most max_iter steps), k_i = (sqrt(m_i^2+xi^2 E_i^2), xi p_i),
  * w_m = xi^(2n-3) sqrt_s prod(|k_i|/k_i^0) / sum(|k_i|^2/k_i^0).
  * d_p: outgoing rows 8.. are read (massless, CM frame) and overwritten; incoming rows untouched.
  * d_w: [N] multiplied in place by w_m.  h_masses: n doubles on the HOST. */
@@ -277,6 +280,23 @@ typedef struct ms_gen_config {
  * d_x1x2: [2][ld] or NULL (pdf only). */
 int ms_generate(const ms_gen_config* cfg, int64_t N, ms_rng rng, const double* d_edges, double* d_p, double* d_w,
                 double* d_x1x2, int64_t ld, uint32_t* d_fail, void* stream);
+
+/* ms_generate_unweight -- ms_generate with the hit-or-miss decision of ms_unweight taken in the same kernel (
+ * reading U): possible whenever w_max is known before the launch, i.e. for every batch after the pre-run.  Beside everything
+ * ms_generate writes, bit (e & 31) of d_accept_bits[e >> 5] is set iff u_e * w_max < w_e, with u_e = Philox uniform j = 0 of
+ * (rng_unweight.seed, rng_unweight.stream, rng_unweight.event_offset + e) -- the decision ms_unweight takes, bit for bit.
+ * d_accept_bits: ms_accept_bits_words(N) = 8 ceil(N/256) uint32, 16-byte aligned, every word is written.  d_wmax: device
+ * scalar, read at kernel start (precondition 0 < w_max < inf, else nothing is accepted).
+ * ms_unweight_compact -- the compaction half of ms_unweight for decisions that already exist as such a bit array: same
+ * outputs (d_idx, d_w_out = max(1, w/w_max), d_rows_out, *d_n_accepted; stable order, `cap` as in ms_unweight), same
+ * scratch (ms_unweight_scratch_bytes(N)); reads 4 bytes per 32 events instead of drawing a uniform per event. */
+size_t ms_accept_bits_words(int64_t N);
+int ms_generate_unweight(const ms_gen_config* cfg, int64_t N, ms_rng rng, const double* d_edges, double* d_p, double* d_w,
+                         double* d_x1x2, int64_t ld, uint32_t* d_fail, const double* d_wmax, ms_rng rng_unweight,
+                         uint32_t* d_accept_bits, void* stream);
+int ms_unweight_compact(int64_t N, const double* d_w, const double* d_wmax, const uint32_t* d_accept_bits, int n_rows,
+                        const double* d_rows_in, int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out,
+                        int64_t* d_n_accepted, void* d_scratch, size_t scratch_bytes, int64_t ld, void* stream);
 
 /* ms_fill_uniforms -- materialise Philox uniforms j = 0..d-1 as rows d_r[d][ld] (step S0 on its own). */
 int ms_fill_uniforms(int64_t N, int d, ms_rng rng, double* d_r, int64_t ld, void* stream);

@@ -24,7 +24,7 @@ _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECU
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_fill_uniforms")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
 
 
 class MadSpaceError(RuntimeError):
@@ -87,6 +87,10 @@ def lib() -> C.CDLL:
         L.ms_reduce_max.argtypes = [_i64, _vp, _vp, _vp]
         L.ms_unweight.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
         L.ms_generate.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp]
+        L.ms_generate_unweight.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp, ms_rng, _vp, _vp]
+        L.ms_unweight_compact.argtypes = [_i64, _vp, _vp, _vp, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
+        L.ms_accept_bits_words.restype = C.c_size_t
+        L.ms_accept_bits_words.argtypes = [_i64]
         _lib = L
     return _lib
 
@@ -210,6 +214,25 @@ def gen_config(n, mapping="fastrambo", sqrt_s=0.0, grid_dims=0, grid_bins=0, pdf
 def ms_generate(cfg: ms_gen_config, N, r: ms_rng, d_edges, d_p, d_w, d_x1x2, ld, d_fail=None, stream=None) -> None:
     _check("ms_generate", lib().ms_generate(C.byref(cfg), N, r, _ptr(d_edges), _ptr(d_p), _ptr(d_w), _ptr(d_x1x2), ld,
                                             _ptr(d_fail), _stream(stream)))
+
+
+def ms_accept_bits_words(N) -> int:
+    return int(lib().ms_accept_bits_words(N))
+
+
+def ms_generate_unweight(cfg: ms_gen_config, N, r: ms_rng, d_edges, d_p, d_w, d_x1x2, ld, d_fail, d_wmax, r_unweight: ms_rng,
+                         d_accept_bits, stream=None) -> None:
+    _check("ms_generate_unweight", lib().ms_generate_unweight(C.byref(cfg), N, r, _ptr(d_edges), _ptr(d_p), _ptr(d_w),
+                                                              _ptr(d_x1x2), ld, _ptr(d_fail), _ptr(d_wmax), r_unweight,
+                                                              _ptr(d_accept_bits), _stream(stream)))
+
+
+def ms_unweight_compact(N, d_w, d_wmax, d_accept_bits, n_rows, d_rows_in, cap, d_idx, d_w_out, d_rows_out, d_n_accepted,
+                        d_scratch, scratch_bytes, ld, stream=None) -> None:
+    _check("ms_unweight_compact", lib().ms_unweight_compact(N, _ptr(d_w), _ptr(d_wmax), _ptr(d_accept_bits), n_rows,
+                                                            _ptr(d_rows_in), cap, _ptr(d_idx), _ptr(d_w_out), _ptr(d_rows_out),
+                                                            _ptr(d_n_accepted), _ptr(d_scratch), scratch_bytes, ld,
+                                                            _stream(stream)))
 
 
 def ms_rambo_massive_reweight(N, n, mapping, sqrt_s, masses: Sequence[float], d_x, r: ms_rng, d_p, d_w, ld,

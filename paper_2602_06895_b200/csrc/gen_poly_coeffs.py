@@ -56,7 +56,7 @@ def main():
             return mp.mpf(1) / 2 + r / 6
         return (mp.expm1(r) - r) / (r * r)
 
-    pe = fit(ge, -rmax, rmax, 12)
+    pe = fit(ge, -rmax, rmax, 10)
     show("PE", pe)
     worst = 0
     for i in range(-2000, 2001):
@@ -82,8 +82,8 @@ def main():
         r = mp.sqrt(z)
         return (mp.cos(mp.pi * r) - 1) / z
 
-    ps = fit(gs, 0, zq, 8)
-    pc = fit(gc, 0, zq, 8)
+    ps = fit(gs, 0, zq, 7)
+    pc = fit(gc, 0, zq, 7)
     show("PS", ps)
     show("PC", pc)
     ws = wc = 0
@@ -110,7 +110,7 @@ def atan_turns():
         t = mp.sqrt(z)
         return mp.atan(t) / (2 * mp.pi * t)
 
-    pa = fit(g, 0, zmax, 12)
+    pa = fit(g, 0, zmax, 11)
     show("PA", pa)
     worst = 0
     for i in range(1, 3001):

@@ -30,11 +30,11 @@ static int grid_for(K kernel, int64_t N, size_t smem)
 #if MS_PART == 0 || MS_PART == 1
 constexpr bool kExact = MS_PART == 1;
 
-template <int MASSMODE, bool PDF, bool TOY, bool ROWS, bool GRID>
+template <int MASSMODE, bool PDF, bool TOY, bool ROWS, int GRID>
 static cudaError_t launch_gen_t(const GenParams& P, cudaStream_t stream)
 {
     auto kernel = gen_kernel<MS_N, kExact, MASSMODE, PDF, TOY, ROWS, GRID>;
-    const size_t smem = GRID ? (size_t)P.grid_dims * P.grid_bins * sizeof(double2) : 0;
+    const size_t smem = GRID != 0 ? (size_t)P.grid_dims * P.grid_bins * sizeof(double2) : 0;
     if (smem > 48 * 1024) {
         cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
@@ -51,19 +51,25 @@ cudaError_t MS_CAT(launch_gen_exact_, MS_N)
     (const GenParams& P, int massmode, bool pdf, bool toy, cudaStream_t stream)
 {
     if (P.x_rows != nullptr)
-        return massmode == 2 ? launch_gen_t<2, false, false, true, false>(P, stream)
-                             : launch_gen_t<0, false, false, true, false>(P, stream);
-    const int sel = (P.grid_dims > 0 ? 4 : 0) | (pdf ? 2 : 0) | (toy ? 1 : 0);
-#define MS_CASE(v)                                                                                                  \
-    case v:                                                                                                         \
-        return massmode == 0   ? launch_gen_t<0, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 4) != 0>(P, stream) \
-               : massmode == 1 ? launch_gen_t<1, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 4) != 0>(P, stream) \
-                               : launch_gen_t<2, ((v) & 2) != 0, ((v) & 1) != 0, false, ((v) & 4) != 0>(P, stream);
+        return massmode == 2 ? launch_gen_t<2, false, false, true, 0>(P, stream)
+                             : launch_gen_t<0, false, false, true, 0>(P, stream);
+    // grid kind: 0 none, 1 any bin count, 6 / 7: 64 / 128 bins (the bin and the in-bin offset come straight from the
+    // Philox mantissa: ms_kernels.cuh, UniformSource)
+    const int gk = P.grid_dims <= 0 ? 0 : (P.grid_bins == 64 ? 2 : P.grid_bins == 128 ? 3 : 1);
+    const int sel = gk * 4 + (pdf ? 2 : 0) + (toy ? 1 : 0);
+#define MS_GK(v) ((v) / 4 == 0 ? 0 : (v) / 4 == 1 ? 1 : (v) / 4 == 2 ? 6 : 7)
+#define MS_CASE(v)                                                                                               \
+    case v:                                                                                                      \
+        return massmode == 0   ? launch_gen_t<0, ((v) & 2) != 0, ((v) & 1) != 0, false, MS_GK(v)>(P, stream)    \
+               : massmode == 1 ? launch_gen_t<1, ((v) & 2) != 0, ((v) & 1) != 0, false, MS_GK(v)>(P, stream)    \
+                               : launch_gen_t<2, ((v) & 2) != 0, ((v) & 1) != 0, false, MS_GK(v)>(P, stream);
     switch (sel) {
         MS_CASE(0) MS_CASE(1) MS_CASE(2) MS_CASE(3) MS_CASE(4) MS_CASE(5) MS_CASE(6) MS_CASE(7)
+        MS_CASE(8) MS_CASE(9) MS_CASE(10) MS_CASE(11) MS_CASE(12) MS_CASE(13) MS_CASE(14) MS_CASE(15)
         default: return cudaErrorInvalidValue;
     }
 #undef MS_CASE
+#undef MS_GK
 }
 #else
 cudaError_t MS_CAT(launch_inverse_, MS_N)(const InvParams& P, bool massive, cudaStream_t stream)

@@ -75,19 +75,20 @@ __device__ __forceinline__ double2 lds_double2(uint32_t addr)
 // ---------------------------------------------------------------------------------------------------
 static __constant__ double c_PL[8] = {0x1.0c97816496c47p-3, 0x1.0fb04d4fa4e54p-3, 0x1.3b1cbf421a439p-3, 0x1.745cf674f6889p-3,
                                       0x1.c71c72078b928p-3, 0x1.249249247343fp-2, 0x1.9999999999a4fp-2, 0x1.5555555555555p-1};
-static __constant__ double c_PE[12] = {0x1.61c2c1ba3877dp-33, 0x1.1f820dbf5e732p-29, 0x1.ae642ad2afd38p-26, 0x1.27e4d2841fc93p-22,
-                                       0x1.71de3a5af94e9p-19, 0x1.a01a01aa828e2p-16, 0x1.a01a01a0195e6p-13, 0x1.6c16c16c158f5p-10,
-                                       0x1.1111111111111p-7,  0x1.5555555555557p-5,  0x1.5555555555555p-3,  0x1.0000000000000p-1};
-// sin(pi r) = r PS(r^2), cos(pi r) = 1 + r^2 PC(r^2) on |r| <= 1/4 (max rel. error 4.9e-17 / 2.9e-17)
-static __constant__ double c_PS[8] = {-0x1.6c4a9959ac7f4p-16, 0x1.e8ee999bfa907p-12, -0x1.e3074b08b3e5dp-8, 0x1.507834859edd7p-4,
-                                      -0x1.32d2cce62aa54p-1,  0x1.466bc6775aad8p+1,  -0x1.4abbce625be53p+2, 0x1.921fb54442d18p+1};
-static __constant__ double c_PC[8] = {0x1.1e688a088894cp-18, -0x1.b6de64b9ca596p-14, 0x1.f9d386d6a8da6p-10, -0x1.a6d1f2a0675b5p-6,
-                                      0x1.e1f506891ad52p-3,  -0x1.55d3c7e3cbff7p+0,  0x1.03c1f081b5ac4p+2,  -0x1.3bd3cc9be45dep+2};
+static __constant__ double c_PE[10] = {0x1.af3ce42b12b24p-26, 0x1.2894f52583578p-22, 0x1.71de0be2b5e96p-19, 0x1.a019b621f9d08p-16,
+                                       0x1.a01a01a83ba17p-13, 0x1.6c16c1794e1dcp-10, 0x1.1111111110918p-7,  0x1.5555555553b6cp-5,
+                                       0x1.5555555555556p-3,  0x1.0000000000001p-1};
+// sin(pi r) = r PS(r^2), cos(pi r) = 1 + r^2 PC(r^2) on |r| <= 1/4 (max rel. error 4.1e-17 / 2.8e-17: seven coefficients
+// each are as accurate as eight -- beyond that the rounding of the coefficients themselves is the limit)
+static __constant__ double c_PS[7] = {0x1.e3da06a519070p-12, -0x1.e3002ae3c4436p-8, 0x1.50782f90efce4p-4, -0x1.32d2cce2a0bd8p-1,
+                                      0x1.466bc67758457p+1,  -0x1.4abbce625be3fp+2, 0x1.921fb54442d18p+1};
+static __constant__ double c_PC[7] = {-0x1.b2dfe0c850620p-14, 0x1.f9cdecb2c924fp-10, -0x1.a6d1eebaf8f4cp-6, 0x1.e1f50686529f0p-3,
+                                      -0x1.55d3c7e3cb0d4p+0,  0x1.03c1f081b5ac0p+2,  -0x1.3bd3cc9be45dep+2};
 
-// atan(t) / (2 pi) = t PA(t^2) on |t| <= sqrt(2) - 1 (max rel. error 6.6e-17)
-static __constant__ double c_PA[12] = {-0x1.7051651483447p-9, 0x1.8a943f5548953p-8, -0x1.065065cdaaeecp-7, 0x1.30dd6cc651060p-7,
-                                       -0x1.5b7a2c88f6247p-7, 0x1.91276be34fb19p-7, -0x1.da1b804092706p-7, 0x1.21bb93a648421p-6,
-                                       -0x1.7483758b589b1p-6, 0x1.04c26be3acccdp-5, -0x1.b2995e7b7b5cep-5, 0x1.45f306dc9c883p-3};
+// atan(t) / (2 pi) = t PA(t^2) on |t| <= sqrt(2) - 1 (max rel. error 1.1e-16)
+static __constant__ double c_PA[11] = {0x1.b5885ec281cd5p-9, -0x1.c422ffbd37433p-8, 0x1.286af929b3851p-7, -0x1.5a412e165d6b3p-7,
+                                       0x1.910a4ffc569efp-7, -0x1.da19c30b5077fp-7, 0x1.21bb8b5affe87p-6, -0x1.7483755d2c2f7p-6,
+                                       0x1.04c26be36ad85p-5, -0x1.b2995e7b7b135p-5, 0x1.45f306dc9c882p-3};
 
 // Horner, coefficients highest degree first.
 template <int NC>
@@ -176,8 +177,8 @@ __device__ __forceinline__ void sincos_2pi(double x, double& sn, double& cs)
     const int q = __double2loint(qm);
     const double r = fma(-0.5, qm - magic, 2.0 * x);
     const double r2 = r * r;
-    const double s = r * horner<8>(c_PS, r2);
-    const double c = fma(r2, horner<8>(c_PC, r2), 1.0);
+    const double s = r * horner<7>(c_PS, r2);
+    const double c = fma(r2, horner<7>(c_PC, r2), 1.0);
     const bool odd = q & 1;
     const double a = odd ? c : s;                               // sin(pi r + q pi/2)
     const double b = odd ? s : c;
@@ -198,7 +199,7 @@ __device__ __forceinline__ double atan2_turns(double y, double x)
     const double num = big ? mn - mx : mn;
     const double den = big ? mn + mx : mx;
     const double t = num * rcp_fast(fmax(den, 0x1p-1000));      // x = y = 0 (no azimuth): turn 0, not NaN
-    double turn = fma(t, horner<12>(c_PA, t * t), big ? 0.125 : 0.0);
+    double turn = fma(t, horner<11>(c_PA, t * t), big ? 0.125 : 0.0);
     if (swap) turn = 0.25 - turn;
     if (x < 0.0) turn = 0.5 - turn;
     if (y < 0.0) turn = 1.0 - turn;
@@ -235,7 +236,7 @@ __device__ __forceinline__ double exp_any(double h)
     const double nd = nm - magic;
     double r = fma(-nd, 0x1.62e42fee00000p-1, h);
     r = fma(-nd, 0x1.a39ef35793c76p-33, r);
-    const double p = fma(r * r, horner<12>(c_PE, r), r);
+    const double p = fma(r * r, horner<10>(c_PE, r), r);
     const double sc = __hiloint2double((n + 1023) << 20, 0);
     return fma(sc, p, sc);
 }
@@ -294,7 +295,7 @@ __device__ __forceinline__ double mass_ratio(double y, double z, double& u, doub
 
 // One FastRambo mass step (Eq. 60, 65; weight factor = Eq. 67 / Eq. 63):
 //   weight factor (k+1)(1 - y^(1/k)) / g_RQF(y) with g_RQF = z (2y + c z) / D^2, D = 1 + (c-2) y z (Eq. 64, 1-y = z)
-//   = (k+1) D^2 / ((2y + c z) S) = wnum / wden   (the z of 1 - y^(1/k) = z/S cancels).
+//   = (k+1) D^2 / ((2y + c z) S) = (k+1) wnum / wden   (the z of 1 - y^(1/k) = z/S cancels).
 template <int K>
 __device__ __forceinline__ void fastrambo_mass_step(double x, double& u, double& omu2, double& wnum, double& wden)
 {
@@ -303,8 +304,16 @@ __device__ __forceinline__ void fastrambo_mass_step(double x, double& u, double&
     rqf_inverse(x, c, y, z);
     const double S = mass_ratio<K>(y, z, u, omu2);
     const double D = fma((c - 2.0) * y, z, 1.0);
-    wnum = (double)(K + 1) * (D * D);
+    wnum = D * D;                                  // the factors (k+1) are multiplied in once: fastrambo_chain_factor
     wden = fma(c, z, 2.0 * y) * S;
+}
+
+// prod_{k=1}^{n-2} (k+1) = (n-1)!: the constant part of the FastRambo weight factors
+__host__ __device__ constexpr double fastrambo_chain_factor(int n)
+{
+    double f = 1.0;
+    for (int k = 1; k <= n - 2; ++k) f *= (double)(k + 1);
+    return f;
 }
 
 // Binomial coefficient at compile time.
@@ -435,18 +444,17 @@ struct Vec4 {
 };
 
 // One two-body decay {Q_{i-1}, M} -> p_{i-1} + Q_i (Eq. 54-55; angles Eq. 25):
-// p has energy e_rest and momentum q in the rest frame of Q (e_rest = q for a massless particle), and is boosted by the
+// p has energy e_rest and momentum q = q2 / 2 in the rest frame of Q (e_rest = q for a massless particle), and is boosted by the
 // pure boost taking (M,0) to Q (reading D-3); the recoil is Q - p.  `first`: Q = (M,0,0,0), no boost needed.
 template <bool FIRST>
-__device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double e_rest, double q, double x_cos, double x_phi,
+__device__ __forceinline__ void two_body_decay(Vec4& Q, double M, double e_rest, double q2, double x_cos, double x_phi,
                                                Vec4& p)
 {
-    const double cth = fma(2.0, x_cos, -1.0);
-    const double sth = 2.0 * sqrt_fast(x_cos * (1.0 - x_cos));   // sqrt(1 - cth^2) without cancellation
+    // q2 = 2q: cos(theta) = 2x - 1 and sin(theta) = 2 sqrt(x (1 - x)) (no cancellation) hand their factor 2 to q
     double sn, cs;
     sincos_2pi(x_phi, sn, cs);
-    const double qs = q * sth;
-    const double rx = qs * cs, ry = qs * sn, rz = q * cth;
+    const double qs = q2 * sqrt_fast(x_cos * (1.0 - x_cos));
+    const double rx = qs * cs, ry = qs * sn, rz = q2 * (x_cos - 0.5);
     if constexpr (FIRST) {
         p.e = e_rest; p.x = rx; p.y = ry; p.z = rz;
         Q.e = M - e_rest; Q.x = -rx; Q.y = -ry; Q.z = -rz;

@@ -37,6 +37,10 @@ struct GenParams {
     double* w;                 // [N]
     double* x1x2;              // [2][ld] or nullptr
     uint32_t* fail;
+    // fused unweighting decision (ms_generate_unweight), or accept_bits == nullptr
+    const double* wmax;        // device scalar
+    uint32_t* accept_bits;     // [8 ceil(N/256)]: bit (e & 31) of word e >> 5 <=> event e accepted
+    PhiloxKey ukey;            // unweighting stream
 };
 
 struct InvParams {

@@ -2,7 +2,8 @@
 tests check).  Marshalling and buffer ownership only: every arithmetic step is a call into the C ABI.
 
 One step = ms_generate (Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [rescale] -> [boost] -> [toy] -> weight)
-           [-> ms_unweight (accept + stable compaction) against w_max of the pre-run, computed once per grid]
+           [unweighting: ms_generate_unweight instead -- the hit-or-miss decision against w_max of the pre-run (computed
+            once per grid) is taken in the generation kernel -- then ms_unweight_compact (stable compaction)]
            [-> ms_fastrambo_inverse -> ms_vegas_map(inverse)]            (round trip, cfg 5)
 """
 from __future__ import annotations
@@ -16,7 +17,8 @@ import torch
 
 from . import (ms_elementwise_max, ms_weight_histogram, ms_wmax_from_histogram, MS_HIST_BINS,
                ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
-               ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID)
+               ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID, ms_generate_unweight,
+               ms_unweight_compact, ms_accept_bits_words)
 
 
 @contextlib.contextmanager
@@ -63,7 +65,8 @@ class PathSpec:
 
 
 class HotPath:
-    def __init__(self, spec: PathSpec, N: int, device="cuda:0", cap: Optional[int] = None, gather_rows: bool = True):
+    def __init__(self, spec: PathSpec, N: int, device="cuda:0", cap: Optional[int] = None, gather_rows: bool = True,
+                 fuse_decision: bool = True):
         if not torch.cuda.is_available():
             raise RuntimeError("HotPath needs a CUDA device: there is no CPU fallback")
         self.spec, self.N, self.device = spec, int(N), torch.device(device)
@@ -94,6 +97,11 @@ class HotPath:
             self._pre = None                                   # buffers of the replayed pre-run, allocated on first use
             self.fail_pre = torch.zeros(1, dtype=torch.int32, device=self.device)
             self._wmax_cached = False                          # w_max is a function of (spec, grid): computed once
+            # fuse_decision: generate() also takes the accept/reject decisions (one bit per event) and unweight() only
+            # compacts; False keeps the two-call form ms_generate + ms_unweight (same results, bit for bit)
+            self.fuse_decision = bool(fuse_decision)
+            self.accept_bits = torch.empty(max(ms_accept_bits_words(self.N), 4), dtype=torch.int32, device=self.device)
+            self._bits_offset = None                           # event offset the bits in accept_bits belong to
         if spec.inverse:
             self.d_inv = 3 * spec.n - 4
             self.x_inv = torch.empty((self.d_inv, self.ld), **f64)
@@ -106,6 +114,7 @@ class HotPath:
             raise MadSpaceError("ms_check_grid", MS_EGRID)
         self.grid_dims, self.grid_bins = h_edges.shape[0], h_edges.shape[1] - 1
         self._wmax_cached = False                              # a new grid changes every weight, hence w_max
+        self._bits_offset = None
         # unused trailing dimensions whose bins all have n_bins * width == 1.0 exactly contribute a Jacobian of exactly 1
         tail = h_edges[self.spec.d_used:]
         self.tail_unit_jacobian = bool(tail.shape[0] > 0 and np.all(self.grid_bins * np.diff(tail, axis=1) == 1.0))
@@ -118,9 +127,20 @@ class HotPath:
 
     # ---- stages -------------------------------------------------------------------------------
     def generate(self, event_offset: int = 0, stream=None) -> None:
+        s = self.spec
+        if s.unweight and self.fuse_decision:
+            self.ensure_wmax(stream)
+            with _on(stream):
+                ms_generate_unweight(self.cfg, self.N, rng(s.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
+                                     self.x1x2, self.ld, self.fail, self.wmax, rng(s.seed_unweight, 1, event_offset),
+                                     self.accept_bits, None)
+            self._bits_offset = event_offset
+            return
         with _on(stream):
-            ms_generate(self.cfg, self.N, rng(self.spec.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
+            ms_generate(self.cfg, self.N, rng(s.seed_events, 0, event_offset), self.d_edges, self.p, self.w,
                         self.x1x2, self.ld, self.fail, None)
+        if s.unweight:
+            self._bits_offset = None
 
     def adapt_grid(self, event_offset: int = 0, alpha: float = 0.5, stream=None) -> np.ndarray:
         """One VEGAS adaptation step from the weights of the last generate(event_offset): accumulate w^2 per bin on the
@@ -165,7 +185,13 @@ class HotPath:
     def unweight(self, event_offset: int = 0, stream=None) -> None:
         s = self.spec
         self.ensure_wmax(stream)
+        rows_n, rows = (s.rows_p, self.p) if self.gather_rows else (0, None)
         with _on(stream):
+            if self.fuse_decision and self._bits_offset == event_offset:
+                # the generation kernel has decided already: count + scatter only
+                ms_unweight_compact(self.N, self.w, self.wmax, self.accept_bits, rows_n, rows, self.cap, self.idx,
+                                    self.w_out, self.rows_out, self.n_acc, self.scratch, self.scratch_bytes, self.ld, None)
+                return
             ms_unweight(self.N, self.w, self.wmax, rng(s.seed_unweight, 1, event_offset), s.rows_p if self.gather_rows else 0,
                         self.p if self.gather_rows else None, self.cap, self.idx, self.w_out, self.rows_out, self.n_acc,
                         self.scratch, self.scratch_bytes, self.ld, None)
@@ -224,7 +250,7 @@ class HotPath:
         """Kernels of this library enqueued by one step in steady state (w_max cached; memsets/copies not counted)."""
         k = 1
         if self.spec.unweight:
-            k += 2                                  # decide / scatter of ms_unweight
+            k += 2                                  # count (or decide) / scatter
         if self.spec.inverse:
             k += 2 if self.d_edges is not None else 1
         return k
