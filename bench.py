@@ -35,11 +35,12 @@ UNIT = "events/s"
 FP64_LANES_PER_SM = 64            # B200 (GB100): 64 FP64 FMA lanes per SM (datasheet 37 TFLOP/s = 148*64*2*1.965 GHz)
 
 # Hand-counted fp64-pipe instructions (DADD/DMUL/DFMA/DSETP) of the final formulas, per stage (DESIGN.md §5
-# "algorithmic op count"; MUFU seeds and int<->fp conversions run on the XU pipe and are not counted here).
+# "algorithmic op count"; MUFU seeds and int<->fp conversions run on the XU pipe and are not counted here).  The counts
+# follow csrc/ms_math.cuh / ms_kernels.cuh line by line; ncu's executed fp64 instructions per event agree to 1-2 %.
 RCP, SQRT, SQRT_H = 3, 5, 7   # third-order correction after the MUFU seed: rcp_fast, sqrt_fast, sqrt_fast with 1/(2 sqrt)
 RQF_INVERSE = 16 + SQRT + RCP  # s, beta, a, discriminant (3), sqrt, d1 (2), a2, product, rcp, y (3), z (3)
-EXP = 18                   # magic-number reduction (4), r^2, degree-11 Horner, 2 fma
-SINCOS = 21                # quarter-turn reduction (4), r^2, two degree-7 Horners, 2
+EXP = 16                   # magic-number reduction (4), r^2, ten-coefficient Horner (9), 2 fma
+SINCOS = 19                # quarter-turn reduction (4), r^2, two seven-coefficient Horners (12), 2
 
 
 def _pow_cost(r):          # multiplications of u^r by squaring
@@ -47,15 +48,17 @@ def _pow_cost(r):          # multiplications of u^r by squaring
 
 
 def _mass_ratio(k):        # v = y^(1/k), u = sqrt(v), 1 - v = z / (1 + v + ... + v^(k-1))
-    if k == 1:
-        return SQRT
     if k == 2:
         return 2 * (SQRT) + 1 + RCP + 1
     return _pow_cost(2 * k) + 4 + RCP + 2 + 1 + (k - 1) + RCP + 1      # Halley root of order 2k, v, S, rcp, 1-v
 
 
-def fast_mass_step(k):     # RQF inverse, ratio, weight factor (k+1) D^2 / ((2y + c z) S), q, M, weight products
-    return RQF_INVERSE + _mass_ratio(k) + (3 if k == 1 else 7) + 5
+def fast_mass_step(k):
+    """k = 1 (c_1 = 2): z = sqrt(1-x), y = x/(1+z), u = sqrt(y), weight factor 1.  k >= 2: RQF inverse, ratio, D (2), D^2,
+    (2y + c z) S (3), two weight products; then q2 = M (1-u^2), e_rest, M u (3)."""
+    if k == 1:
+        return 1 + SQRT + 1 + RCP + 1 + SQRT + 3
+    return RQF_INVERSE + _mass_ratio(k) + 2 + 1 + 3 + 2 + 3
 
 
 def exact_mass_step(k):
@@ -66,13 +69,24 @@ def exact_mass_step(k):
     return 1 + 3 * k + 16 + 1 + SQRT + 3
 
 
-ALG_FP64 = {"uniform": 1, "vegas_dim": 5, "decay_first": 3 + SQRT + 1 + SINCOS + 4 + 1,
-            "decay": 3 + SQRT + 1 + SINCOS + 4 + 2 + RCP + 4 + 4 + 3 + 4,
-            "toy_pair": 13, "weight": 5 + RCP + 3 + 3, "pdf": 2 * EXP + 4 + RCP + 2 + 4 + 3 + 4, "boost_particle": 4,
-            "rescale_start": 1 + RCP + 1 + 1 + SQRT, "rescale_eval_massive": 2 + SQRT_H + 4, "rescale_eval_massless": 2,
-            "rescale_eval_fixed": 2 + RCP + 1, "rescale_final_massive": 2 + SQRT_H + 4 + 3, "rescale_final_massless": 5,
-            "rescale_weight": 3 + 3 + RCP}
-RESCALE_EVALUATIONS = 4    # cfg4 converges in <= 3 Newton steps: 4 evaluations of F
+# decay: x(1-x) (2), sqrt, q2 sqrt, sincos, rx ry (2), x - 1/2 and rz (2) [first: recoil energy (1)];
+# boost: Q0 + M, M (Q0 + M), rcp, energy (4 + 2), factor (3), three components, recoil (4)
+DECAY_REST = 2 + SQRT + 1 + SINCOS + 2 + 2
+ALG_FP64 = {"uniform": 1, "vegas_dim_pow2": 4, "vegas_dim_generic": 6, "decay_first": DECAY_REST + 1,
+            "decay": DECAY_REST + 2 + RCP + 6 + 3 + 3 + 4,
+            "toy_pair": 13, "weight": 9, "weight_toy": 2, "pdf": 2 * EXP + 23, "boost_particle": 4,
+            "rescale_start": 3 + RCP + 2 + SQRT + 1, "rescale_halley_massive": 2 + SQRT_H + 4 + 4, "rescale_eval_massive": 2 + SQRT_H + 4,
+            "rescale_eval_massless": 3, "rescale_halley_step": 8 + RCP, "rescale_final_massive": 5, "rescale_final_massless": 1,
+            "rescale_weight": 6 + RCP, "rescale_momenta": 3}
+RESCALE_HALLEY_STEPS = 2   # cfg4: two Halley steps from xi_0 reach 1e-14 W for every event; the third evaluation is the output
+
+
+def grid_dims_used(wl: ms_inputs.Workload) -> int:
+    """Grid dimensions the kernel actually looks up: unused trailing dimensions of a uniform power-of-two grid carry a
+    Jacobian of exactly 1 and are skipped (reading X-3, ms_gen_config.tail_unit_jacobian)."""
+    if wl.grid_dims == 0:
+        return 0
+    return wl.d_ps if wl.grid_kind == "uniform" else wl.grid_dims
 
 
 def alg_bytes_per_event(wl: ms_inputs.Workload) -> int:
@@ -99,23 +113,28 @@ PHILOX_IMAD_WIDE = 20                  # 32x32 -> 64-bit multiplies per Philox4x
 
 def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
     n = wl.n
-    c = ALG_FP64["uniform"] * wl.d + ALG_FP64["vegas_dim"] * wl.grid_dims
+    gd = grid_dims_used(wl)
+    pow2 = wl.grid_bins in (64, 128)
+    c = ALG_FP64["uniform"] * (wl.d_ps if gd == 0 else 0) + (ALG_FP64["vegas_dim_pow2"] if pow2 else ALG_FP64["vegas_dim_generic"]) * gd
     for i in range(2, n):
         c += fast_mass_step(n - i) if wl.mapping == "fastrambo" else exact_mass_step(n - i)
     c += ALG_FP64["decay_first"] + ALG_FP64["decay"] * (n - 2)
     if wl.toy:
-        c += ALG_FP64["toy_pair"] * (n - 1)
+        c += ALG_FP64["toy_pair"] * (n - 1) + ALG_FP64["weight_toy"]
     if wl.pdf:
         c += ALG_FP64["pdf"] + ALG_FP64["boost_particle"] * n
     if wl.masses and wl.massive_mode == "reweight":
-        # per decay: 1-u via rcp (2 + RCP), factorised Kallen (7) + sqrt, 1/(2M) (RCP + 1), q, e_rest (4), weight (5), M_i (1)
+        # per decay: 1-u via rcp (2 + RCP), factorised Kallen (7) + sqrt, 1/M (RCP + 1), q, e_rest (4), weight (5), M_i (1)
         c += (n - 1) * (2 + RCP + 7 + SQRT + RCP + 1 + 1 + 4 + 5 + 1) + 2
     elif wl.masses:
         nm = sum(1 for m in wl.masses if m > 0)
-        c += ALG_FP64["rescale_start"] + ALG_FP64["rescale_weight"]
-        c += RESCALE_EVALUATIONS * (ALG_FP64["rescale_eval_massive"] * nm + ALG_FP64["rescale_eval_massless"] * (n - nm)
-                                    + ALG_FP64["rescale_eval_fixed"])
+        c += ALG_FP64["rescale_start"] + ALG_FP64["rescale_weight"] + ALG_FP64["rescale_momenta"] * n
+        c += RESCALE_HALLEY_STEPS * (ALG_FP64["rescale_halley_massive"] * nm + ALG_FP64["rescale_eval_massless"] * (n - nm)
+                                     + ALG_FP64["rescale_halley_step"])
+        c += ALG_FP64["rescale_eval_massive"] * nm + ALG_FP64["rescale_eval_massless"] * (n - nm) + 1
         c += ALG_FP64["rescale_final_massive"] * nm + ALG_FP64["rescale_final_massless"] * (n - nm)
+    if wl.unweight:
+        c += 3                              # fused decision: uniform conversion, u * w_max, comparison
     return c + ALG_FP64["weight"]
 
 
@@ -317,12 +336,13 @@ def stage_roofline(name, wl, N, t_ms, peaks, n_accepted=0, d_inv=0, traffic=None
                                                              ("rescale" if wl.massive_mode == "rescale" else "reweight") if wl.masses else "massless",
                                                              ",pdf" if wl.pdf else "", ",toy" if wl.toy else "", ",grid" if wl.grid_dims else "")}
     elif name == "unweight":
-        nbytes = 8 * N + n_accepted * 16 * (rows_p + 2)
-        sides = {"hbm": nbytes / hbm, "imad": N * PHILOX_IMAD_WIDE / (peaks["imad_wide_ginst_measured"] * 1e9)}
-        extra = {"alg_bytes": nbytes, "alg_imad_wide_per_event": PHILOX_IMAD_WIDE,
-                 "kernel": "ms::unweight_decide_kernel + ms::unweight_scatter_kernel",
-                 "note": "SURVEY 8(d)'s 8 B/event read stream, and the quarter-rate integer-multiply pipe of the one Philox call "
-                         "per decision (20 IMAD.WIDE): the larger of the two is the ceiling"}
+        # what is left of the unweighting after ms_generate_unweight has taken the decisions: one bit per event to read,
+        # the accepted events to gather -- two short dependent kernels, launch / latency bound (see unweighting_total)
+        nbytes = N // 8 + n_accepted * (8 + 16 * (rows_p + 2))
+        sides = {"hbm": nbytes / hbm}
+        extra = {"alg_bytes": nbytes, "kernel": "ms::unweight_count_kernel + ms::unweight_scatter_kernel",
+                 "note": "compaction only (the accept/reject decisions are taken inside ms::gen_kernel): a few MB behind two "
+                         "dependent launches, latency bound; the cost of the whole unweighting is in unweighting_total"}
     elif name == "fastrambo_inverse":
         nbytes = N * (32 * wl.n + 8 * d_inv + 8)
         sides = {"hbm": nbytes / hbm, "alu": N * alg_fp64_inverse(wl.n) / fp64}
@@ -341,6 +361,35 @@ def stage_roofline(name, wl, N, t_ms, peaks, n_accepted=0, d_inv=0, traffic=None
     out.update({"%s_time_ms" % k: 1e3 * v for k, v in sides.items()})
     out.update(extra)
     return out
+
+
+def unweighting_total(torch, hp, wl, N, stage_ms, peaks, offset, reps=5):
+    """The whole cost of the unweighting in a step: what the fused decision adds to the generation kernel (the same
+    launch timed with and without it) plus the compaction stage, against SURVEY.md section 8(d)'s roofline for it (an
+    8 B/event read stream: 21 us at 2^24 events) and against the integer-multiply pipe time of one Philox call per
+    decision (20 IMAD.WIDE, measured rate)."""
+    def gen_ms(fused):
+        hp.fuse_decision = fused
+        hp.generate(offset)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record()
+        for _ in range(reps):
+            hp.generate(offset)
+        ev[1].record()
+        torch.cuda.synchronize()
+        return ev[0].elapsed_time(ev[1]) / reps
+    try:
+        t_plain, t_fused = gen_ms(False), gen_ms(True)
+    finally:
+        hp.fuse_decision = True
+    total = max(t_fused - t_plain, 0.0) + stage_ms["unweight"]
+    t_hbm = 1e3 * 8 * N / (peaks["hbm_gbs"] * 1e9)
+    t_imad = 1e3 * N * PHILOX_IMAD_WIDE / (peaks["imad_wide_ginst_measured"] * 1e9)
+    return {"generate_with_decision_ms": t_fused, "generate_without_decision_ms": t_plain, "compaction_stage_ms": stage_ms["unweight"],
+            "total_ms": total, "hbm_time_ms_8B_per_event": t_hbm, "imad_time_ms_20_per_event": t_imad,
+            "frac_of_larger_side": max(t_hbm, t_imad) / total if total > 0 else None,
+            "note": "SURVEY 8(d): 8 B/event read stream; one Philox call per decision = 20 IMAD.WIDE on the integer-multiply pipe"}
 
 
 def time_steps(torch, hp, steps, warmup, first_offset, stride, barrier):
@@ -466,6 +515,7 @@ def measure_config(torch, ms, name, steps, warmup, peaks, oracle_seconds):
         out["note"] = "sub-wave batch: launch-latency bound, reported, not a roofline target"
     if wl.unweight:
         out["unweighted_events_per_s"] = n_acc * steps / t_total
+        out["unweighting_total"] = unweighting_total(torch, hp, wl, N, stage_ms, peaks, 0)
     out["parity"] = parity_and_pins(torch, ms, hp, wl, name)
     if oracle_seconds > 0:
         cb, _ = time_oracle(wl, target_seconds=oracle_seconds, per_core=False)
@@ -666,6 +716,7 @@ def run_ours(args):
                 "traffic": g["traffic"], "parity": parity_and_pins(torch, ms, hp, wl, wl.name), "cpu_baseline": cb}
         if wl.unweight:
             head["unweighted_events_per_s"] = sum(counts) * args.steps / t_total
+            head["unweighting_total"] = unweighting_total(torch, hp, wl, N, stage_ms, peaks, 0)
         per_config[wl.name] = head
         del hp
         torch.cuda.empty_cache()

@@ -246,6 +246,11 @@ int ms_histogram_fill(int64_t N, const double* d_obs, const double* d_w, double 
  *   unweighted against the final maximum w_f by ms_unweight applied to max(w, w_old) (ms_elementwise_max) with a
  *   fresh uniform stream: an event kept with probability min(1, w/w_old) survives with min(1, max(w, w_old)/w_f). */
 #define MS_HIST_BINS 32768
+/* ms_gather (bookkeeping of the kept events, no arithmetic on the data): d_out[r*ld_out + k] = d_in[r*ld_in + d_idx[k]] for
+ * r < n_rows, k < K (8-byte words copied bit for bit: doubles, or int64 viewed as such), and, if d_idx_out != NULL,
+ * d_idx_out[k] = d_idx[k] + idx_add (local -> global event index).  Pointers 8-byte aligned; d_out must not overlap d_in. */
+int ms_gather(int64_t K, const int64_t* d_idx, int n_rows, const double* d_in, int64_t ld_in, double* d_out, int64_t ld_out,
+              int64_t idx_add, int64_t* d_idx_out, void* stream);
 int ms_weight_histogram(int64_t N, const double* d_w, uint64_t* d_counts, void* stream);
 int ms_wmax_from_histogram(const uint64_t* h_counts, double fraction, double* h_wmax);
 int ms_elementwise_max(int64_t N, const double* d_a, const double* d_b, double* d_out, void* stream);

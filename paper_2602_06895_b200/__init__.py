@@ -24,7 +24,7 @@ _ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECU
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_gather", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
 
 
 class MadSpaceError(RuntimeError):
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         L.ms_weight_histogram.argtypes = [_i64, _vp, _vp, _vp]
         L.ms_wmax_from_histogram.argtypes = [_vp, _dbl, _vp]
         L.ms_elementwise_max.argtypes = [_i64, _vp, _vp, _vp, _vp]
+        L.ms_gather.argtypes = [_i64, _vp, _int, _vp, _i64, _vp, _i64, _i64, _vp, _vp]
         L.ms_vegas_accumulate.argtypes = [_i64, _int, _int, _vp, ms_rng, _vp, _vp]
         L.ms_vegas_refine.argtypes = [_int, _int, _vp, _dbl, _vp, _vp]
         L.ms_vegas_map.argtypes = [_i64, _int, _int, _vp, _int, _vp, ms_rng, _vp, _vp, _i64, _vp]
@@ -292,6 +293,11 @@ def ms_wmax_from_histogram(h_counts, fraction) -> float:
 
 def ms_elementwise_max(N, d_a, d_b, d_out, stream=None) -> None:
     _check("ms_elementwise_max", lib().ms_elementwise_max(N, _ptr(d_a), _ptr(d_b), _ptr(d_out), _stream(stream)))
+
+
+def ms_gather(K, d_idx, n_rows, d_in, ld_in, d_out, ld_out, idx_add=0, d_idx_out=None, stream=None) -> None:
+    _check("ms_gather", lib().ms_gather(K, _ptr(d_idx), n_rows, _ptr(d_in), ld_in, _ptr(d_out), ld_out, idx_add,
+                                        _ptr(d_idx_out), _stream(stream)))
 
 
 def ms_chili(N, n, s_lab, masses, pt_min, y_cut, d_x, r: ms_rng, d_p, d_w, d_x1x2, ld, stream=None) -> None:

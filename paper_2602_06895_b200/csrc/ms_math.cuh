@@ -32,6 +32,22 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// The same with the round keys given (ms_params.h, PhiloxRoundKeys: launch parameters in the constant bank).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxRoundKeys& rk,
+                                              uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ rk.k[2 * round];
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ rk.k[2 * round + 1];
+        c3 = lo0;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
 // u = (2*(W>>12)+1) * 2^-53 with W = hi<<32 | lo: the 52 bits are OR-ed into the mantissa of 1.0 giving
 // 1 + m 2^-52; subtracting (1 - 2^-53) leaves (2m+1) 2^-53, which is representable, so the one DADD is exact and
 // no int->fp conversion is needed (reading R-3).
@@ -247,10 +263,10 @@ __device__ __forceinline__ double exp_any(double h)
 // z = (beta + sqrt(beta^2 + 4s(1+beta))) / (2(1+beta)), s = 1-x, beta = (c-2)s.  Since b = 2 + beta the two
 // discriminants are the same number, so one square root and one reciprocal give both roots, every term positive.
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void rqf_inverse(double x, double c, double& y, double& z)
+__device__ __forceinline__ void rqf_inverse(double x, double c_minus_2, double& y, double& z)
 {
     const double s = 1.0 - x;
-    const double beta = (c - 2.0) * s;
+    const double beta = c_minus_2 * s;
     const double a = 1.0 + beta;
     const double sq = sqrt_fast(fma(beta, beta, 4.0 * s * a));
     const double d1 = (a + 1.0) + sq;
@@ -266,6 +282,12 @@ __device__ __forceinline__ constexpr double table1_ck(int k)
     return k == 1 ? 2.0 : k == 2 ? 2.712001 : k == 3 ? 3.084521 : k == 4 ? 3.313073 : k == 5 ? 3.467512
          : k == 6 ? 3.578833 : 3.662872;
 }
+// The same numbers and c_k - 2 in the constant bank (index k): a 64-bit literal costs two moves into uniform registers
+// at every use, a constant-bank operand none.
+static __constant__ double c_CK[8] = {0.0, table1_ck(1), table1_ck(2), table1_ck(3), table1_ck(4), table1_ck(5), table1_ck(6),
+                                      table1_ck(7)};
+static __constant__ double c_CKM2[8] = {0.0, table1_ck(1) - 2.0, table1_ck(2) - 2.0, table1_ck(3) - 2.0, table1_ck(4) - 2.0,
+                                        table1_ck(5) - 2.0, table1_ck(6) - 2.0, table1_ck(7) - 2.0};
 
 // v = y^(1/K) and u = sqrt(v) = y^(1/(2K)) (Eq. 60), and 1 - v = z / (1 + v + ... + v^(K-1)) from
 // z = 1 - y (exact factorisation: no cancellation, no logarithm).  Returns S = 1 + v + ... + v^(K-1).
@@ -299,20 +321,31 @@ __device__ __forceinline__ double mass_ratio(double y, double z, double& u, doub
 template <int K>
 __device__ __forceinline__ void fastrambo_mass_step(double x, double& u, double& omu2, double& wnum, double& wden)
 {
-    constexpr double c = table1_ck(K);
+    if constexpr (K == 1) {
+        // c_1 = 2 (Table 1): Eq. 64 becomes r = 1 - (1-y)^2, the map coincides with RamboOnDiet's and the
+        // weight factor is exactly 1: z = sqrt(1-x), y = x / (1 + z), u = sqrt(y), nothing else
+        const double z = sqrt_fast(1.0 - x);
+        u = sqrt_fast(x * rcp_fast(1.0 + z));
+        omu2 = z;
+        wnum = 1.0;
+        wden = 1.0;
+        return;
+    }
+    const double c = c_CK[K], cm2 = c_CKM2[K];
     double y, z;
-    rqf_inverse(x, c, y, z);
+    rqf_inverse(x, cm2, y, z);
     const double S = mass_ratio<K>(y, z, u, omu2);
-    const double D = fma((c - 2.0) * y, z, 1.0);
+    const double D = fma(cm2 * y, z, 1.0);
     wnum = D * D;                                  // the factors (k+1) are multiplied in once: fastrambo_chain_factor
     wden = fma(c, z, 2.0 * y) * S;
 }
 
-// prod_{k=1}^{n-2} (k+1) = (n-1)!: the constant part of the FastRambo weight factors
+// prod_{k=2}^{n-2} (k+1) = (n-1)!/2: the constant part of the FastRambo weight factors of the steps k >= 2 (the k = 1
+// step's factor, (k+1)(1-y)/g_RQF with c_1 = 2, is exactly 1 as a whole)
 __host__ __device__ constexpr double fastrambo_chain_factor(int n)
 {
     double f = 1.0;
-    for (int k = 1; k <= n - 2; ++k) f *= (double)(k + 1);
+    for (int k = 2; k <= n - 2; ++k) f *= (double)(k + 1);
     return f;
 }
 

@@ -13,6 +13,22 @@ struct PhiloxKey {
     uint64_t event_offset;
 };
 
+// The ten round keys of a Philox4x32-10 call, (k0 + r W0, k1 + r W1) for r = 0..9 (Weyl sequence of the key, reading R-1):
+// they depend on the seed alone, so the host works them out once and the generation kernels read them as constant-bank
+// operands of the XORs (in the kernel the additions were re-done per 256-event tile: 18 instructions per event).
+struct PhiloxRoundKeys {
+    uint32_t k[20];
+};
+inline PhiloxRoundKeys philox_round_keys(uint32_t k0, uint32_t k1)
+{
+    PhiloxRoundKeys rk;
+    for (int r = 0; r < 10; ++r) {
+        rk.k[2 * r] = k0 + (uint32_t)r * 0x9E3779B9u;
+        rk.k[2 * r + 1] = k1 + (uint32_t)r * 0xBB67AE85u;
+    }
+    return rk;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Launch parameters (plain data, passed by value as a __grid_constant__).
 // ---------------------------------------------------------------------------------------------------
@@ -41,6 +57,7 @@ struct GenParams {
     const double* wmax;        // device scalar
     uint32_t* accept_bits;     // [8 ceil(N/256)]: bit (e & 31) of word e >> 5 <=> event e accepted
     PhiloxKey ukey;            // unweighting stream
+    PhiloxRoundKeys rk, urk;   // round keys of key / ukey (filled by the dispatcher)
 };
 
 struct InvParams {

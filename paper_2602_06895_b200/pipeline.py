@@ -18,7 +18,7 @@ import torch
 from . import (ms_elementwise_max, ms_weight_histogram, ms_wmax_from_histogram, MS_HIST_BINS,
                ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
                ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID, ms_generate_unweight,
-               ms_unweight_compact, ms_accept_bits_words)
+               ms_unweight_compact, ms_accept_bits_words, ms_gather)
 
 
 @contextlib.contextmanager
@@ -263,17 +263,75 @@ class HotPath:
 class RunningUnweighter:
     """Unweighting against a running maximum weight with an overweight allowance (reading U-2),
     batch by batch on the device: exact weight histogram -> w_max on the host (32768 counts) -> partial unweighting of
-    the batch (ms_unweight) -> kept (global index, weight, w_max at the time); finalize() re-unweights the kept events
-    against the final maximum.  Marshalling and buffer ownership only: every arithmetic step is a library call."""
+    the batch (ms_unweight) -> kept (global index, weight, w_max at the time, rows); finalize() re-unweights the kept
+    events against the final maximum.  Every buffer is allocated once; every step that touches data is a library call
+    (ms_weight_histogram, ms_unweight, ms_gather, ms_elementwise_max) or a plain copy / fill; the host reads one count
+    per batch and the 256 KB histogram through pinned memory."""
 
-    def __init__(self, fraction: float, seed: int, device="cuda:0", n_rows: int = 0):
+    def __init__(self, fraction: float, seed: int, device="cuda:0", n_rows: int = 0, batch_cap: int = 1 << 20,
+                 kept_cap: int = 1 << 20):
         self.fraction, self.seed, self.device = float(fraction), int(seed), torch.device(device)
-        self.counts = torch.zeros(MS_HIST_BINS, dtype=torch.int64, device=self.device)
+        self.n_rows = int(n_rows)
+        f64 = dict(dtype=torch.float64, device=self.device)
+        i64 = dict(dtype=torch.int64, device=self.device)
+        self.counts = torch.zeros(MS_HIST_BINS, **i64)
+        self.h_counts = torch.zeros(MS_HIST_BINS, dtype=torch.int64).pin_memory()
+        self.d_wmax = torch.zeros(2, **f64)
+        self.h_wmax = torch.zeros(2, dtype=torch.float64).pin_memory()
+        self.n_acc = torch.zeros(2, **i64)
+        self.h_nacc = torch.zeros(2, dtype=torch.int64).pin_memory()
         self.w_max = 0.0
         self.trace = []
-        self.kept_idx, self.kept_w, self.kept_old, self.kept_rows = [], [], [], []
-        self.n_rows = n_rows
+        self.fill = 0                                        # kept events so far
+        self._alloc_batch(int(batch_cap))
+        self._alloc_kept(int(kept_cap))
 
+    # ---- buffers ---------------------------------------------------------------------------------
+    def _alloc_batch(self, cap: int) -> None:
+        cap = (cap + 1) // 2 * 2
+        f64 = dict(dtype=torch.float64, device=self.device)
+        self.batch_cap = cap
+        self.b_idx = torch.empty(cap, dtype=torch.int64, device=self.device)
+        self.b_wout = torch.empty(cap, **f64)
+        self.b_rows = torch.empty((self.n_rows, cap), **f64) if self.n_rows > 0 else None
+        self.scratch_bytes = ms_unweight_scratch_bytes(cap)
+        self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
+
+    def _alloc_kept(self, cap: int) -> None:
+        cap = (cap + 1) // 2 * 2
+        f64 = dict(dtype=torch.float64, device=self.device)
+        i64 = dict(dtype=torch.int64, device=self.device)
+        old = (self.kept_idx, self.kept_w, self.kept_old, self.kept_rows) if self.fill > 0 else None
+        self.kept_cap = cap
+        self.kept_idx = torch.empty(cap, **i64)
+        self.kept_w = torch.empty(cap, **f64)
+        self.kept_old = torch.empty(cap, **f64)
+        self.kept_rows = torch.empty((self.n_rows, cap), **f64) if self.n_rows > 0 else None
+        self.w_eff = torch.empty(cap, **f64)
+        self.fin = torch.empty(cap, **i64)
+        self.f_wout = torch.empty(cap, **f64)
+        self.f_idx = torch.empty(cap, **i64)
+        self.f_rows = torch.empty((self.n_rows, cap), **f64) if self.n_rows > 0 else None
+        self.f_scratch_bytes = ms_unweight_scratch_bytes(cap)
+        self.f_scratch = torch.empty(self.f_scratch_bytes, dtype=torch.uint8, device=self.device)
+        if old is not None:                                  # growth: plain copies of what was kept
+            k = self.fill
+            self.kept_idx[:k].copy_(old[0][:k])
+            self.kept_w[:k].copy_(old[1][:k])
+            self.kept_old[:k].copy_(old[2][:k])
+            if self.n_rows > 0:
+                self.kept_rows[:, :k].copy_(old[3][:, :k])
+
+    def _read_count(self) -> int:
+        self.h_nacc.copy_(self.n_acc, non_blocking=True)
+        torch.cuda.current_stream(self.device).synchronize()
+        return int(self.h_nacc[0])
+
+    def _set_wmax(self, value: float) -> None:
+        self.h_wmax[0] = value
+        self.d_wmax.copy_(self.h_wmax, non_blocking=True)
+
+    # ---- batches ----------------------------------------------------------------------------------
     def add_batch(self, w: torch.Tensor, N: int, event_offset: int, rows: Optional[torch.Tensor] = None, ld: int = 0,
                   stream=None) -> int:
         with _on(stream):
@@ -281,54 +339,59 @@ class RunningUnweighter:
 
     def _add_batch(self, w, N, event_offset, rows, ld) -> int:
         stream = None                                        # torch's current stream (set by add_batch)
+        if N > self.batch_cap:
+            self._alloc_batch(N)
+        # (1) the exact histogram of all weights so far -> the running maximum (host walk over 32768 counts)
         ms_weight_histogram(N, w, self.counts, stream)
-        self.w_max = max(self.w_max, ms_wmax_from_histogram(self.counts.cpu().numpy(), self.fraction))
+        self.h_counts.copy_(self.counts, non_blocking=True)
+        torch.cuda.current_stream(self.device).synchronize()
+        self.w_max = max(self.w_max, ms_wmax_from_histogram(self.h_counts.numpy(), self.fraction))
         self.trace.append(self.w_max)
-        f64 = dict(dtype=torch.float64, device=self.device)
-        d_wmax = torch.tensor([self.w_max], **f64)
-        cap = N
-        idx = torch.empty(cap, dtype=torch.int64, device=self.device)
-        w_out = torch.empty(cap, **f64)
-        n_acc = torch.zeros(1, dtype=torch.int64, device=self.device)
-        sb = ms_unweight_scratch_bytes(N)
-        scratch = torch.empty(sb, dtype=torch.uint8, device=self.device)
+        self._set_wmax(self.w_max)
+        # (2) partial unweighting of the batch against it
         use_rows = rows is not None and self.n_rows > 0
-        rows_out = torch.empty((self.n_rows, cap), **f64) if use_rows else None
-        ms_unweight(N, w, d_wmax, rng(self.seed, 1, event_offset), self.n_rows if use_rows else 0, rows if use_rows else None,
-                    cap, idx, w_out, rows_out, n_acc, scratch, sb, ld if use_rows else N, stream)
-        k = int(n_acc.item())
-        self.kept_idx.append(idx[:k] + event_offset)
-        self.kept_w.append(w[idx[:k]])                       # gather of the kept weights (indexing, no arithmetic)
-        self.kept_old.append(torch.full((k,), self.w_max, **f64))
+        ms_unweight(N, w, self.d_wmax, rng(self.seed, 1, event_offset), self.n_rows if use_rows else 0,
+                    rows if use_rows else None, self.batch_cap, self.b_idx, self.b_wout, self.b_rows if use_rows else None,
+                    self.n_acc, self.scratch, self.scratch_bytes, ld if use_rows else N, stream)
+        k = self._read_count()
+        if k == 0:
+            return 0
+        if self.fill + k > self.kept_cap:
+            self._alloc_kept(max(2 * self.kept_cap, self.fill + k))
+        # (3) append: kept weight = w[idx], global index = idx + offset (one ms_gather), w_max at the time, rows
+        f = self.fill
+        ms_gather(k, self.b_idx, 1, w, 0, self.kept_w[f:], self.kept_cap - f, event_offset, self.kept_idx[f:], stream)
+        self.kept_old[f:f + k].fill_(self.w_max)
         if use_rows:
-            self.kept_rows.append(rows_out[:, :k])
+            self.kept_rows[:, f:f + k].copy_(self.b_rows[:, :k])
+        self.fill = f + k
         return k
 
     def finalize(self, stream=None):
-        """Returns (global indices, output weights, rows or None) of the finally unweighted events."""
+        """Returns (global indices, output weights, rows or None) of the finally unweighted events (views of buffers this
+        object owns: copy them before the next finalize())."""
         with _on(stream):
             return self._finalize()
 
     def _finalize(self):
         stream = None                                        # torch's current stream (set by finalize)
-        f64 = dict(dtype=torch.float64, device=self.device)
-        idx_all = torch.cat(self.kept_idx) if self.kept_idx else torch.empty(0, dtype=torch.int64, device=self.device)
-        K = idx_all.numel()
+        K = self.fill
         if K == 0:
-            return idx_all, torch.empty(0, **f64), None
-        pad = K + (K & 1)
-        w_all, old_all = torch.zeros(pad, **f64), torch.zeros(pad, **f64)
-        w_all[:K] = torch.cat(self.kept_w)
-        old_all[:K] = torch.cat(self.kept_old)
-        w_eff = torch.empty(pad, **f64)
-        ms_elementwise_max(K, w_all, old_all, w_eff, stream)
-        d_wmax = torch.tensor([self.w_max], **f64)
-        fin = torch.empty(K, dtype=torch.int64, device=self.device)
-        w_out = torch.empty(K, **f64)
-        n_acc = torch.zeros(1, dtype=torch.int64, device=self.device)
-        sb = ms_unweight_scratch_bytes(K)
-        scratch = torch.empty(sb, dtype=torch.uint8, device=self.device)
-        ms_unweight(K, w_eff, d_wmax, rng(self.seed, 2, 0), 0, None, K, fin, w_out, None, n_acc, scratch, sb, pad, stream)
-        k = int(n_acc.item())
-        rows = torch.cat(self.kept_rows, dim=1)[:, fin[:k]] if self.kept_rows else None
-        return idx_all[fin[:k]], w_out[:k], rows
+            return self.f_idx[:0], self.f_wout[:0], None
+        # an event kept with probability min(1, w/w_old) survives with min(1, max(w, w_old)/w_f): the same hit-or-miss
+        # test on max(w, w_old) with a fresh uniform stream (stream 2, counter = position in the kept list)
+        ms_elementwise_max(K, self.kept_w, self.kept_old, self.w_eff, stream)
+        self._set_wmax(self.w_max)
+        ms_unweight(K, self.w_eff, self.d_wmax, rng(self.seed, 2, 0), 0, None, self.kept_cap, self.fin, self.f_wout, None,
+                    self.n_acc, self.f_scratch, self.f_scratch_bytes, self.kept_cap, stream)
+        k = self._read_count()
+        if k == 0:
+            return self.f_idx[:0], self.f_wout[:0], None
+        # global indices (int64 copied as 8-byte words) and rows of the survivors
+        ms_gather(k, self.fin, 1, self.kept_idx.view(torch.float64), 0, self.f_idx.view(torch.float64), self.kept_cap, 0, None,
+                  stream)
+        rows = None
+        if self.n_rows > 0:
+            ms_gather(k, self.fin, self.n_rows, self.kept_rows, self.kept_cap, self.f_rows, self.kept_cap, 0, None, stream)
+            rows = self.f_rows[:, :k]
+        return self.f_idx[:k], self.f_wout[:k], rows
