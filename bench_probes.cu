@@ -51,6 +51,25 @@ __global__ void __launch_bounds__(kBlock) probe_write_kernel(int64_t N, int rows
     }
 }
 
+// Dependent DFMA chain, `chains` independent chains per thread (1, 2, 4 or 8), launched with ONE warp per block: the time per
+// DFMA of a single warp = the dependent-issue latency (chains = 1) and how many chains a scheduler needs to hide it.
+template <int CH>
+__global__ void probe_dfma_latency_kernel(int iters, double* sink)
+{
+    double a[CH];
+#pragma unroll
+    for (int i = 0; i < CH; ++i) a[i] = threadIdx.x * 1e-3 + i;
+    const double m = 0.999999, c = 1e-7;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < CH; ++i) a[i] = fma(a[i], m, c);
+    }
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < CH; ++i) acc += a[i];
+    sink[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 // KIND: 0 none, 1 LOP3 (alu pipe), 2 IMAD (32-bit), 3 IMAD.WIDE.U32, 4 FFMA, 5 MUFU.RCP (fp32), 6 F2I + I2F (fp64 <-> s32),
 //       7 LDS.64, 8 IADD3, 9 MUFU.RCP64H
 template <int KIND, int K, int ND>
@@ -139,6 +158,20 @@ int probe_write(int64_t N, int rows, double* d_out, int64_t ld, void* stream)
     const int64_t blocks = (N + kBlock - 1) / kBlock;
     const int grid = (int)(blocks < (int64_t)sms * 8 ? blocks : (int64_t)sms * 8);
     probe_write_kernel<<<grid, kBlock, 0, (cudaStream_t)stream>>>(N, rows, d_out, ld);
+    return (int)cudaGetLastError();
+}
+
+// one warp per block, `blocks` blocks; chains = independent DFMA chains per thread
+int probe_dfma_latency(int chains, int blocks, int iters, double* d_sink, void* stream)
+{
+    cudaStream_t s = (cudaStream_t)stream;
+    switch (chains) {
+        case 1: probe_dfma_latency_kernel<1><<<blocks, 32, 0, s>>>(iters, d_sink); break;
+        case 2: probe_dfma_latency_kernel<2><<<blocks, 32, 0, s>>>(iters, d_sink); break;
+        case 4: probe_dfma_latency_kernel<4><<<blocks, 32, 0, s>>>(iters, d_sink); break;
+        case 8: probe_dfma_latency_kernel<8><<<blocks, 32, 0, s>>>(iters, d_sink); break;
+        default: return (int)cudaErrorInvalidValue;
+    }
     return (int)cudaGetLastError();
 }
 

@@ -48,6 +48,7 @@ def lib() -> C.CDLL:
         L.probe_dfma3.argtypes = [i, i, vp, vp]
         L.probe_write.argtypes = [i64, i, vp, i64, vp]
         L.probe_mix.argtypes = [i, i, i, i, i, vp, vp]
+        L.probe_dfma_latency.argtypes = [i, i, i, vp, vp]
         _lib = L
     return _lib
 
@@ -156,6 +157,33 @@ def issue_model(torch) -> dict:
     return out
 
 
+def dfma_latency(torch) -> dict:
+    """Cycles per DFMA of ONE warp per SM with 1, 2, 4, 8 independent chains per thread (dependent-issue latency and the
+    parallelism needed to hide it), at the maximum SM clock."""
+    s = torch.cuda.current_stream().cuda_stream
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    iters = 1 << 16
+    sink = torch.empty(sms * 32, dtype=torch.float64, device="cuda")
+    try:
+        q = subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"],
+                           capture_output=True, text=True).stdout.strip().splitlines()[0]
+        clock_hz = float(q) * 1e6
+    except Exception:
+        clock_hz = 1965e6
+    out = {"clock_mhz_assumed": clock_hz / 1e6}
+    for ch in (1, 2, 4, 8):
+        _check(lib().probe_dfma_latency(ch, sms, iters, sink.data_ptr(), s), "probe_dfma_latency")
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(5):
+            _check(lib().probe_dfma_latency(ch, sms, iters, sink.data_ptr(), s), "probe_dfma_latency")
+        ev1.record()
+        ev1.synchronize()
+        out["cycles_per_dfma_%d_chains" % ch] = ev0.elapsed_time(ev1) * 1e-3 / 5 * clock_hz / (iters * ch)
+    return out
+
+
 def unweight_density(torch, steps: int = 20, warmup: int = 3) -> dict:
     """ms_unweight alone on 2^24 synthetic weights x 24 momentum rows at several acceptance rates -- the unweighting
     efficiencies a production run sees after grid adaptation rather than the 1e-4 of the seeded-grid
@@ -240,7 +268,7 @@ def main() -> int:
     if what == "fp64":
         res = {"probe": "fp64", "const_operand": fp64_rate(torch, 2.0), "three_registers": fp64_rate(torch, 2.0, True)}
     elif what == "issue-model":
-        res = {"probe": "issue-model", **issue_model(torch)}
+        res = {"probe": "issue-model", **issue_model(torch), "dfma_latency": dfma_latency(torch)}
     elif what == "unweight-density":
         res = unweight_density(torch)
     elif what == "chili":

@@ -57,6 +57,24 @@ def test_roofline_inputs_follow_the_workloads():
     assert c["cfg1"] < c["cfg2"] < c["cfg5"] and c["cfg4rw"] < c["cfg4"]
 
 
+def test_design_roofline_table_is_the_bench_functions():
+    """DESIGN.md section 5 quotes bytes and fp64 instructions per event for every config; they are bench.py's functions, not a
+    copy that can drift (the two disagreed)."""
+    import re
+    sys.path.insert(0, ROOT)
+    import bench
+    text = open(os.path.join(ROOT, "DESIGN.md")).read()
+    rows = re.findall(r"^\| (cfg\w+) \([^|]*\|[^|]*\| (\d+) \| (\d+) \|", text, flags=re.M)
+    seen = {}
+    for name, nbytes, ninst in rows:
+        seen[name] = (int(nbytes), int(ninst))
+    assert set(seen) == set(ms_inputs.WORKLOADS), seen
+    for name, (nbytes, ninst) in seen.items():
+        wl = ms_inputs.WORKLOADS[name]
+        assert nbytes == bench.alg_bytes_per_event(wl), name
+        assert ninst == bench.alg_fp64_per_event(wl), name
+
+
 import pytest
 
 
