@@ -386,7 +386,9 @@ def unweighting_total(torch, hp, wl, N, stage_ms, peaks, offset, reps=5):
     total = max(t_fused - t_plain, 0.0) + stage_ms["unweight"]
     t_hbm = 1e3 * 8 * N / (peaks["hbm_gbs"] * 1e9)
     t_imad = 1e3 * N * PHILOX_IMAD_WIDE / (peaks["imad_wide_ginst_measured"] * 1e9)
+    t_roof = 1e3 * max(N * alg_bytes_per_event(wl) / (peaks["hbm_gbs"] * 1e9), N * (alg_fp64_per_event(wl) - 3) / (peaks["fp64_ginst_measured"] * 1e9))
     return {"generate_with_decision_ms": t_fused, "generate_without_decision_ms": t_plain, "compaction_stage_ms": stage_ms["unweight"],
+            "generation_frac_without_decision": t_roof / t_plain if t_plain > 0 else None,
             "total_ms": total, "hbm_time_ms_8B_per_event": t_hbm, "imad_time_ms_20_per_event": t_imad,
             "frac_of_larger_side": max(t_hbm, t_imad) / total if total > 0 else None,
             "note": "SURVEY 8(d): 8 B/event read stream; one Philox call per decision = 20 IMAD.WIDE on the integer-multiply pipe"}
