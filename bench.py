@@ -141,10 +141,13 @@ def alg_fp64_per_event(wl: ms_inputs.Workload) -> int:
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu captures (recorded, not measured by
 # this script; --traffic overrides the headline's): {workload: {stage: (bytes, source)}}.
 NCU_TRAFFIC = {
-    "cfg2": {"generate": (3.295350e9 + 513.28e3, "profiles/r01e_final.md"), "unweight": (134.25e6 + 3.9e6 + 7.7e6, "profiles/r01e_final.md")},
-    "cfg3": {"generate": (16.583720e9 + 112.1e3, "profiles/r01e_final.md")},
-    "cfg4": {"generate": (6.651895e9 + 172.5e3, "profiles/r01e_final.md")},
-    "cfg5": {"generate": (5.443808e9 + 91e3, "profiles/r01e_final.md"), "vegas_inverse": (2.684e9 + 2.638e9, "profiles/r01e_final.md")},
+    "cfg2": {"generate": (3.297553e9 + 75e3, "profiles/r02a_round_summary.md"), "unweight": (2.104e6 + 7.545e6, "profiles/r02a_round_summary.md")},
+    "cfg3": {"generate": (16.583559e9 + 386e3, "profiles/r02a_round_summary.md")},
+    "cfg4": {"generate": (6.650893e9 + 22e3, "profiles/r02a_round_summary.md")},
+    "cfg4rw": {"generate": (6.651803e9 + 35e3, "profiles/r02a_round_summary.md")},
+    "cfg5": {"generate": (5.445426e9 + 104e3, "profiles/r02a_round_summary.md"),
+             "fastrambo_inverse": (4.296001e9 + 2.780350e9, "profiles/r02a_round_summary.md"),
+             "vegas_inverse": (2.684514e9 + 2.636950e9, "profiles/r02a_round_summary.md")},
 }
 
 # Closed forms of BASELINE.md section 2 (Eq. 81 and the quadratures pinned in tests/test_oracle_phasespace.py): what the

@@ -110,6 +110,29 @@ def test_batches_beyond_the_32_bit_event_index_are_rejected(ms):
     assert _code(ms, ms.ms_generate, cfg, big, r0, None, FAKE, FAKE, None, big + 1, None, 0) == ms.MS_EINVAL
 
 
+def test_fused_unweighting_entry_points_validate_on_the_host(ms):
+    r0, ru = ms.rng(1), ms.rng(3, 1)
+    cfg = ms.gen_config(4, "fastrambo", 1000.0, toy=True)
+    # the decision needs w_max and a bit array; a non-zero reserved field of either rng is rejected
+    assert _code(ms, ms.ms_generate_unweight, cfg, 8, r0, None, FAKE, FAKE, None, 8, None, FAKE, ru, None, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_generate_unweight, cfg, 8, r0, None, FAKE, FAKE, None, 8, None, None, ru, FAKE, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_generate_unweight, cfg, 8, r0, None, FAKE, FAKE, None, 8, None, FAKE, ms.ms_rng(3, 1, 7, 0), FAKE, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_generate_unweight, cfg, 8, r0, None, FAKE, FAKE, None, 1 << 33, None, FAKE, ru, FAKE, 0) == ms.MS_EINVAL   # ld >= 2^32
+    # one ballot word per 32 events, in whole 256-event tiles
+    assert [ms.ms_accept_bits_words(n) for n in (0, 1, 256, 257, 1 << 24)] == [0, 8, 8, 16, 1 << 19]
+    # compaction: bits required, scratch as for ms_unweight
+    assert _code(ms, ms.ms_unweight_compact, 1 << 20, FAKE, FAKE, None, 0, None, 16, FAKE, FAKE, None, FAKE, FAKE,
+                 ms.ms_unweight_scratch_bytes(1 << 20), 1 << 20, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_unweight_compact, 1 << 20, FAKE, FAKE, FAKE, 0, None, 16, FAKE, FAKE, None, FAKE, FAKE, 64,
+                 1 << 20, 0) == ms.MS_EINVAL
+    # gather: row stride of the output must hold K entries; NULL index list
+    assert _code(ms, ms.ms_gather, 10, FAKE, 2, FAKE, 100, FAKE, 5, 0, None, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_gather, 10, None, 2, FAKE, 100, FAKE, 10, 0, None, 0) == ms.MS_EINVAL
+    ms.ms_gather(0, None, 2, None, 0, None, 0, 0, None, 0)
+    # the VEGAS inverse runs in place or on disjoint buffers, never on partially overlapping ones
+    assert _code(ms, ms.ms_vegas_map, 1000, 5, 64, FAKE, 1, 0x100000, r0, 0x100000 + 4096, None, 1000, 0) == ms.MS_EINVAL
+
+
 def test_empty_batches_are_no_ops(ms):
     r0 = ms.rng(1)
     ms.ms_fastrambo(0, 4, 1000.0, None, None, r0, FAKE, FAKE, 0, None, 0)
