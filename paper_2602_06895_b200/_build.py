@@ -68,6 +68,8 @@ def _build_locked(verbose: bool) -> str:
         for part in (0, 1, 2):
             jobs.append((os.path.join(CSRC, "ms_inst.cu"), os.path.join(BUILD, "ms_inst_n%d_p%d.o" % (n, part)),
                          ["-DMS_N=%d" % n, "-DMS_PART=%d" % part]))
+    import time
+    t0 = time.time()
     with cf.ThreadPoolExecutor(max_workers=min(len(jobs), max(os.cpu_count() or 4, 4))) as ex:
         objs = list(ex.map(_compile, jobs))
     tmp = LIB + ".tmp.%d" % os.getpid()
@@ -77,6 +79,8 @@ def _build_locked(verbose: bool) -> str:
         raise RuntimeError("link failed: %s\n%s" % (r.stdout, r.stderr))
     os.replace(tmp, LIB)
     if verbose:
+        print("compiled %d translation units from source with %s %s in %.0f s" % (len(jobs), _nvcc(), " ".join(NVCC_FLAGS[:5]),
+                                                                                 time.time() - t0))
         print("built", LIB)
     return LIB
 
