@@ -359,6 +359,8 @@ def stage_roofline(name, wl, N, t_ms, peaks, n_accepted=0, d_inv=0, traffic=None
         return None
     bound = max(sides, key=sides.get)
     t_roof = sides[bound]
+    if name == "unweight":
+        bound = "latency"                  # two dependent launches over ~2 MB: nowhere near any throughput roofline
     out = {"ms": t_ms, "bound": bound, "roofline_ms": 1e3 * t_roof, "frac": 1e3 * t_roof / t_ms if t_ms > 0 else None,
            "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None}
     out.update({"%s_time_ms" % k: 1e3 * v for k, v in sides.items()})

@@ -123,9 +123,13 @@ def test_per_config_block_covers_every_config_and_stage():
         want = {"generate"} | ({"unweight"} if name in ("cfg2", "cfg5") else set()) \
             | ({"fastrambo_inverse", "vegas_inverse"} if name == "cfg5" else set())
         assert set(c["stages"]) == want, (name, set(c["stages"]))
-        for st in c["stages"].values():
+        for sname, st in c["stages"].items():
             for k in STAGE_KEYS:
                 assert k in st
+            assert st["bound"] in (("latency",) if sname == "unweight" else ("hbm", "alu"))
+        if "unweight" in c["stages"]:
+            ut = c["unweighting_total"]
+            assert ut["total_ms"] > 0 and 0 < ut["frac_of_larger_side"] < 1.5 and ut["generate_with_decision_ms"] > 0
         par = c["parity"]
         assert par["max_dp_over_sqrt_s"] <= 1e-12 and par["fail_count"] == 0
         mc = par["mc_mean_over_closed_form"]
