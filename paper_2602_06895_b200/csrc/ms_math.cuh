@@ -67,6 +67,15 @@ __device__ __forceinline__ void philox_uniform_pair(const PhiloxKey& key, uint64
     b = uniform_from_words(w[2], w[3]);
 }
 
+__device__ __forceinline__ void philox_uniform_pair(const PhiloxRoundKeys& rk, uint32_t stream, uint64_t event, uint32_t pair,
+                                                    double& a, double& b)
+{
+    uint32_t w[4];
+    philox4x32_10((uint32_t)event, (uint32_t)(event >> 32), pair, stream, rk, w);
+    a = uniform_from_words(w[0], w[1]);
+    b = uniform_from_words(w[2], w[3]);
+}
+
 // Clamp of a non-negative double into [2^-53, 1 - 2^-53] on its bit pattern (non-negative doubles order like
 // their high words): same result as fmin(fmax(x, 2^-53), 1 - 2^-53) for 0 <= x <= 1 at half the instructions.
 __device__ __forceinline__ double clamp_open_unit(double x)
@@ -223,7 +232,8 @@ __device__ __forceinline__ double atan2_turns(double y, double x)
 }
 
 // ---------------------------------------------------------------------------------------------------
-// ln(y) for y in (0,1] (normal).  y = m 2^e, m in [sqrt(1/2), sqrt(2)), f = m - 1, s = f/(2+f),
+// ln(y) for positive normal y (callers pass (0,1] or, Chili Eq. 74, [1, 2^511)).  y = m 2^e, m in [sqrt(1/2), sqrt(2)),
+// f = m - 1, s = f/(2+f),
 // ln m = f - s (f - s^2 PL(s^2)).
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double log_unit(double y)

@@ -73,9 +73,11 @@ struct InvParams {
 struct ChiliParams {
     int64_t N, ld;
     PhiloxKey key;
+    PhiloxRoundKeys rk;        // round keys of `key`
     const double* x_rows;      // [3n-2][ld] uniforms, or nullptr -> Philox in-kernel
-    double s_lab, sqrt_s;
-    double weight_unit;        // (2 pi)^(4-3n) * 2 / s_lab
+    double s_lab, sqrt_s, half_sqrt_s, inv_half_sqrt_s;
+    double weight_unit;        // (2 pi)^(4-3n) * 2 / s_lab * pi^(n-1) * prod_{i<n-1} (constant factor of dpT^2/dr: Eq. 72
+                               // 1/pTmin^2 - 1/pTmax^2, Eq. 73 2 (2 lambda + pTmax))
     double inv_ptmax2;         // 1 / pT_max^2, pT_max = sqrt(s_lab)/2 (Eq. 71)
     double masses[kMaxN];
     double inv_ptmin2[kMaxN];  // 1 / pT_min^2 (Eq. 72) or 0 -> Eq. 73
