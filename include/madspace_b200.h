@@ -52,7 +52,8 @@ enum {
     MS_EINVAL = -1,   /* null / misaligned pointer, N <= 0, n out of range, ld < N, bad flag */
     MS_EGRID = -2,    /* reported by ms_check_grid: edges not strictly increasing, x_0 != 0 or x_nb != 1 */
     MS_EKIN = -3,     /* sum of masses >= sqrt_s, tau_min outside (0,1), sqrt_s <= 0 with no per-event array */
-    MS_ECUDA = -4     /* kernel launch failed */
+    MS_ECUDA = -4,    /* kernel launch failed */
+    MS_ELIMIT = -5    /* size beyond the fixed capacity of an entry point that allocates nothing (ms_unweight_static) */
 };
 
 /* Counter-based RNG coordinates, passed by value (reading R-2). */
@@ -202,6 +203,25 @@ size_t ms_unweight_scratch_bytes(int64_t N);
 int ms_unweight(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, int n_rows, const double* d_rows_in,
                 int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted,
                 void* d_scratch, size_t scratch_bytes, int64_t ld, void* stream);
+
+/* ms_unweight_static -- ms_unweight for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments without d_scratch / scratch_bytes, same kernels, same results bit for
+ * bit.  The scratch is a static device array inside the library, MS_UNWEIGHT_STATIC_SCRATCH_BYTES = 2 293 760 B (2.2 MiB),
+ * which every GPU that loads the library holds until the process exits; it serves N <= MS_UNWEIGHT_STATIC_MAX_EVENTS = 2^24
+ * events per call (the largest unweighting batch of the BASELINE.json configs).  N beyond that: MS_ELIMIT, nothing is
+ * enqueued -- split the batch or use ms_unweight.  The call makes no cudaMalloc / cudaFree and calls no allocating
+ * library routine; the first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device,
+ * with the caller's current device) and returns MS_ECUDA if that fails -- under stream capture make one call (N = 0
+ * suffices) before the capture begins.
+ * EVERY call on a device shares the one array: two calls whose kernels can overlap on the GPU (different streams, or
+ * different host threads) race on it and corrupt each other's result -- serialise them on one stream, or give all but one
+ * of them ms_unweight with its own scratch.  The array keeps the previous call's contents; nothing in it has to start at
+ * zero (the decide kernel writes every word the scatter kernel reads), so no clearing is done. */
+#define MS_UNWEIGHT_STATIC_MAX_EVENTS ((int64_t)1 << 24)
+#define MS_UNWEIGHT_STATIC_SCRATCH_BYTES 2293760
+int ms_unweight_static(int64_t N, const double* d_w, const double* d_wmax, ms_rng rng, int n_rows, const double* d_rows_in,
+                       int64_t cap, int64_t* d_idx, double* d_w_out, double* d_rows_out, int64_t* d_n_accepted, int64_t ld,
+                       void* stream);
 
 /* ms_invariant_map -- analytic 1-D mappings for invariants (Eq. 15-20): flat (Eq. 20), power law with
  * exponent nu = par (Eq. 18; par == 1 selects the logarithmic limit Eq. 19; m2 may be the negative auxiliary mass of

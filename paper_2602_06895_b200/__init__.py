@@ -19,12 +19,13 @@ from typing import Optional, Sequence
 from . import _build
 
 MS_MAX_N = 9
-MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA = 0, -1, -2, -3, -4
-_ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA"}
+MS_OK, MS_EINVAL, MS_EGRID, MS_EKIN, MS_ECUDA, MS_ELIMIT = 0, -1, -2, -3, -4, -5
+_ERR = {MS_EINVAL: "MS_EINVAL", MS_EGRID: "MS_EGRID", MS_EKIN: "MS_EKIN", MS_ECUDA: "MS_ECUDA", MS_ELIMIT: "MS_ELIMIT"}
+MS_UNWEIGHT_STATIC_MAX_EVENTS = 1 << 24
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_gather", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_unweight_static", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_gather", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
 
 
 class MadSpaceError(RuntimeError):
@@ -87,6 +88,7 @@ def lib() -> C.CDLL:
         L.ms_toy_integrand.argtypes = [_i64, _int, _dbl, _vp, _vp, _int, _i64, _vp]
         L.ms_reduce_max.argtypes = [_i64, _vp, _vp, _vp]
         L.ms_unweight.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
+        L.ms_unweight_static.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _i64, _vp]
         L.ms_generate.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp]
         L.ms_generate_unweight.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp, ms_rng, _vp, _vp]
         L.ms_unweight_compact.argtypes = [_i64, _vp, _vp, _vp, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
@@ -195,6 +197,13 @@ def ms_unweight(N, d_w, d_wmax, r: ms_rng, n_rows, d_rows_in, cap, d_idx, d_w_ou
     _check("ms_unweight", lib().ms_unweight(N, _ptr(d_w), _ptr(d_wmax), r, n_rows, _ptr(d_rows_in), cap, _ptr(d_idx),
                                             _ptr(d_w_out), _ptr(d_rows_out), _ptr(d_n_accepted), _ptr(d_scratch),
                                             scratch_bytes, ld, _stream(stream)))
+
+
+def ms_unweight_static(N, d_w, d_wmax, r: ms_rng, n_rows, d_rows_in, cap, d_idx, d_w_out, d_rows_out, d_n_accepted, ld,
+                       stream=None) -> None:
+    _check("ms_unweight_static", lib().ms_unweight_static(N, _ptr(d_w), _ptr(d_wmax), r, n_rows, _ptr(d_rows_in), cap,
+                                                          _ptr(d_idx), _ptr(d_w_out), _ptr(d_rows_out), _ptr(d_n_accepted),
+                                                          ld, _stream(stream)))
 
 
 def gen_config(n, mapping="fastrambo", sqrt_s=0.0, grid_dims=0, grid_bins=0, pdf=False, tau_min=0.0, masses=(),
