@@ -6,6 +6,7 @@ library: the kernels live in bench_probes.cu and build into libms_bench_probes.s
     python bench_probes.py issue-model       # 4 DFMA + K other instructions per loop: which pipes issue beside the fp64 pipe
     python bench_probes.py unweight-density  # ms_unweight alone at acceptance rates 1e-4 .. 1
     python bench_probes.py chili             # ms_chili n = 3, 4, 6 at 2^24 events (CUDA events; ncu-able)
+    python bench_probes.py vegas-map         # stand-alone ms_vegas_map, forward and inverse, at the cfg-5 shape
 
 Each prints one JSON line.
 """
@@ -260,6 +261,53 @@ def chili(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) -> dict
     return {"probe": "chili", "events": N, "steps": steps, "results": out}
 
 
+def vegas_map(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) -> dict:
+    """The stand-alone ms_vegas_map at the cfg-5 shape -- 20 dimensions x 2^24 events, 128 seeded bins: forward
+    from uniform rows (16 B per value), forward from in-kernel Philox (8 B per value), inverse (16 B per value)."""
+    sys.path.insert(0, ROOT)
+    import ms_inputs
+    import paper_2602_06895_b200 as ms
+    ms.lib()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    N, d, nb = 1 << 24, 20, 128
+    edges = torch.from_numpy(ms_inputs.seeded_grid(d, nb)).to(dev)
+    r = torch.empty((d, N), dtype=torch.float64, device=dev)
+    x = torch.empty((d, N), dtype=torch.float64, device=dev)
+    jac = torch.empty(N, dtype=torch.float64, device=dev)
+    ms.ms_fill_uniforms(N, d, ms.rng(1, 0, 0), r, N)
+    cases = {
+        "forward_rows": (lambda: ms.ms_vegas_map(N, d, nb, edges, 0, r, ms.rng(0), x, jac, N), 8 * (2 * d + 1) * N),
+        "forward_philox": (lambda: ms.ms_vegas_map(N, d, nb, edges, 0, None, ms.rng(1, 0, 0), x, jac, N), 8 * (d + 1) * N),
+        "inverse": (lambda: ms.ms_vegas_map(N, d, nb, edges, 1, x, ms.rng(0), r, None, N), 8 * 2 * d * N),
+        "inverse_jac": (lambda: ms.ms_vegas_map(N, d, nb, edges, 1, x, ms.rng(0), r, jac, N), 8 * (2 * d + 1) * N),
+    }
+    out = []
+    for name, (call, nbytes) in cases.items():
+        for _ in range(warmup):
+            call()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(steps):
+            call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        ms_call = ev[0].elapsed_time(ev[1]) / steps
+        row = {"case": name, "ms": ms_call, "alg_bytes": nbytes, "achieved_gbs": nbytes / ms_call / 1e6}
+        if hbm_gbs > 0:
+            row["frac_of_hbm"] = row["achieved_gbs"] / hbm_gbs
+        out.append(row)
+    return {"probe": "vegas-map", "events": N, "dims": d, "bins": nb, "steps": steps, "results": out}
+
+
+def _hbm_peak() -> float:
+    pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        with open(pk) as f:
+            return float(json.load(f)["hbm_gbs"])
+    return 0.0
+
+
 def main() -> int:
     import torch
     if not torch.cuda.is_available():
@@ -272,12 +320,9 @@ def main() -> int:
     elif what == "unweight-density":
         res = unweight_density(torch)
     elif what == "chili":
-        hbm = 0.0
-        pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
-        if os.path.exists(pk):
-            with open(pk) as f:
-                hbm = float(json.load(f)["hbm_gbs"])
-        res = chili(torch, hbm_gbs=hbm)
+        res = chili(torch, hbm_gbs=_hbm_peak())
+    elif what == "vegas-map":
+        res = vegas_map(torch, hbm_gbs=_hbm_peak())
     else:
         raise SystemExit("unknown probe: " + what)
     print(json.dumps(res))
