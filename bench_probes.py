@@ -7,6 +7,7 @@ library: the kernels live in bench_probes.cu and build into libms_bench_probes.s
     python bench_probes.py unweight-density  # ms_unweight alone at acceptance rates 1e-4 .. 1
     python bench_probes.py chili             # ms_chili n = 3, 4, 6 at 2^24 events (CUDA events; ncu-able)
     python bench_probes.py vegas-map         # stand-alone ms_vegas_map, forward and inverse, at the cfg-5 shape
+    python bench_probes.py entry-points      # the other stand-alone section-8(b) calls at 2^24 events, each against its own bytes
 
 Each prints one JSON line.
 """
@@ -300,6 +301,70 @@ def vegas_map(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) -> 
     return {"probe": "vegas-map", "events": N, "dims": d, "bins": nb, "steps": steps, "results": out}
 
 
+def entry_points(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) -> dict:
+    """Every stand-alone entry point of SURVEY.md section 8(b) that bench.py does not time as a stage of its own, at 2^24
+    events, against ITS algorithmic bytes (rows read + rows written, 8 B each): the fused path never calls these, a
+    stage-by-stage user does."""
+    sys.path.insert(0, ROOT)
+    import paper_2602_06895_b200 as ms
+    ms.lib()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    N = 1 << 24
+
+    def buf(rows):
+        return torch.empty((rows, N), dtype=torch.float64, device=dev)
+    cases = []
+    # S0
+    r8 = buf(8)
+    cases.append(("ms_fill_uniforms d=8", lambda: ms.ms_fill_uniforms(N, 8, ms.rng(1, 0, 0), r8, N), 8 * 8))
+    # S2/S3/S4 stand-alone: n = 4 FastRambo (8 uniforms) and n = 5 exact Rambo (11 uniforms), rows and Philox
+    p4, w = buf(24), torch.empty(N, dtype=torch.float64, device=dev)
+    ms.ms_fill_uniforms(N, 8, ms.rng(1, 0, 0), r8, N)
+    cases.append(("ms_fastrambo n=4 rows", lambda: ms.ms_fastrambo(N, 4, 1000.0, None, r8, ms.rng(0), p4, w, N), 8 * (8 + 24 + 1)))
+    cases.append(("ms_fastrambo n=4 philox", lambda: ms.ms_fastrambo(N, 4, 1000.0, None, None, ms.rng(1, 0, 0), p4, w, N), 8 * (24 + 1)))
+    r11, p5 = buf(11), buf(28)
+    ms.ms_fill_uniforms(N, 11, ms.rng(1, 0, 0), r11, N)
+    cases.append(("ms_rambo_massless n=5 rows", lambda: ms.ms_rambo_massless(N, 5, 1000.0, None, r11, ms.rng(0), p5, w, N), 8 * (11 + 28 + 1)))
+    cases.append(("ms_rambo_massless n=5 philox", lambda: ms.ms_rambo_massless(N, 5, 1000.0, None, None, ms.rng(1, 0, 0), p5, w, N), 8 * (28 + 1)))
+    # S5: rescale of the n = 4 event in place (16 outgoing rows + w read and written); the input is regenerated each call
+    # outside the timed loop's accounting would hide nothing: the call is timed alone on an already massive event, whose
+    # Newton iteration converges at once -- so time it on fresh massless input by alternating with ms_fastrambo and
+    # subtracting that call's own time (reported as "ms_massive_rescale n=4 (net)")
+    cases.append(("ms_fastrambo n=4 philox, sqrt_s=2000 (feeds the rescale)",
+                  lambda: ms.ms_fastrambo(N, 4, 2000.0, None, None, ms.rng(1, 0, 0), p4, w, N), 8 * (24 + 1)))
+    cases.append(("ms_fastrambo + ms_massive_rescale n=4",
+                  lambda: (ms.ms_fastrambo(N, 4, 2000.0, None, None, ms.rng(1, 0, 0), p4, w, N),
+                           ms.ms_massive_rescale(N, 4, 2000.0, [173.0, 173.0, 0.0, 0.0], 1e-14, 20, p4, w, N)), 8 * (24 + 1) + 8 * 2 * (16 + 1)))
+    # S6: Bjorken x, both phases (n = 5)
+    x1x2, shat, jac = buf(2), torch.empty(N, dtype=torch.float64, device=dev), torch.empty(N, dtype=torch.float64, device=dev)
+    tau_min = (200.0 / 13600.0) ** 2
+    cases.append(("ms_pdf_x_boost sample (philox)", lambda: ms.ms_pdf_x_boost(N, 5, 13600.0 ** 2, tau_min, 0, None, ms.rng(1, 0, 0), x1x2, shat, jac, None, N), 8 * 4))
+    cases.append(("ms_pdf_x_boost boost n=5", lambda: ms.ms_pdf_x_boost(N, 5, 13600.0 ** 2, tau_min, 1, None, ms.rng(0), x1x2, None, None, p5, N), 8 * (2 + 2 * 2 * 5 + 8)))   # reads x1, x2 and (E, pz) of five momenta, writes those back and the two incoming momenta
+    # S7, S8 helpers
+    f = torch.empty(N, dtype=torch.float64, device=dev)
+    cases.append(("ms_toy_integrand n=4", lambda: ms.ms_toy_integrand(N, 4, 100.0, p4, f, False, N), 8 * (16 + 1)))
+    wmax = torch.zeros(1, dtype=torch.float64, device=dev)
+    cases.append(("ms_reduce_max", lambda: ms.ms_reduce_max(N, w, wmax), 8))
+    out = []
+    for name, call, bytes_per_event in cases:
+        for _ in range(warmup):
+            call()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(steps):
+            call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        ms_call = ev[0].elapsed_time(ev[1]) / steps
+        row = {"case": name, "ms": ms_call, "alg_bytes_per_event": bytes_per_event,
+               "achieved_gbs": bytes_per_event * N / ms_call / 1e6}
+        if hbm_gbs > 0:
+            row["frac_of_hbm"] = row["achieved_gbs"] / hbm_gbs
+        out.append(row)
+    return {"probe": "entry-points", "events": N, "steps": steps, "results": out}
+
+
 def _hbm_peak() -> float:
     pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk):
@@ -323,6 +388,8 @@ def main() -> int:
         res = chili(torch, hbm_gbs=_hbm_peak())
     elif what == "vegas-map":
         res = vegas_map(torch, hbm_gbs=_hbm_peak())
+    elif what == "entry-points":
+        res = entry_points(torch, hbm_gbs=_hbm_peak())
     else:
         raise SystemExit("unknown probe: " + what)
     print(json.dumps(res))
