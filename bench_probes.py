@@ -8,6 +8,7 @@ library: the kernels live in bench_probes.cu and build into libms_bench_probes.s
     python bench_probes.py chili             # ms_chili n = 3, 4, 6 at 2^24 events (CUDA events; ncu-able)
     python bench_probes.py vegas-map         # stand-alone ms_vegas_map, forward and inverse, at the cfg-5 shape
     python bench_probes.py entry-points      # the other stand-alone section-8(b) calls at 2^24 events, each against its own bytes
+    python bench_probes.py next-rows         # observables, cuts, histograms, grid accumulation, ... (the NEXT rows), likewise
 
 Each prints one JSON line.
 """
@@ -365,6 +366,57 @@ def entry_points(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) 
     return {"probe": "entry-points", "events": N, "steps": steps, "results": out}
 
 
+def next_rows(torch, steps: int = 20, warmup: int = 3, hbm_gbs: float = 0.0) -> dict:
+    """The calls built beyond section 8(a) (NEXT-2 .. NEXT-4: observables, cuts, histograms, grid accumulation, weight
+    histogram, running maximum, Chili from uniform rows) at 2^24 events, each against its own algorithmic bytes."""
+    sys.path.insert(0, ROOT)
+    import paper_2602_06895_b200 as ms
+    ms.lib()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    N, n = 1 << 24, 4
+
+    def buf(*shape):
+        return torch.empty(shape, dtype=torch.float64, device=dev)
+    p, w, obs = buf(4 * (n + 2), N), buf(N), buf(N)
+    ms.ms_fastrambo(N, n, 1000.0, None, None, ms.rng(1, 0, 0), p, w, N)
+    w2 = w.clone()
+    cases = []
+    for kind, rows in (("PT", 2), ("Y", 2), ("ETA", 3), ("PHI", 2), ("DR", 6), ("MASS", 8)):
+        cases.append(("ms_observable %s" % kind, (lambda k=kind: ms.ms_observable(N, k, 2, 3, n, p, obs, N)), 8 * (rows + 1)))
+    cases.append(("ms_observable HT (n_out = 4)", lambda: ms.ms_observable(N, "HT", 0, 0, n, p, obs, N), 8 * (4 * n + 1)))
+    ms.ms_observable(N, "PT", 2, 3, n, p, obs, N)
+    cases.append(("ms_cut", lambda: ms.ms_cut(N, obs, 20.0, float("inf"), w2), 8 * 3))
+    sw, sw2 = torch.zeros(102, dtype=torch.float64, device=dev), torch.zeros(102, dtype=torch.float64, device=dev)
+    cases.append(("ms_histogram_fill 100 bins", lambda: ms.ms_histogram_fill(N, obs, w, 0.0, 500.0, 100, sw, sw2), 8 * 2))
+    hist = torch.zeros((8, 128), dtype=torch.float64, device=dev)
+    cases.append(("ms_vegas_accumulate 128 x 8", lambda: ms.ms_vegas_accumulate(N, 8, 128, w, ms.rng(1, 0, 0), hist), 8))
+    counts = torch.zeros(32768, dtype=torch.int64, device=dev)      # MS_HIST_BINS
+    cases.append(("ms_weight_histogram", lambda: ms.ms_weight_histogram(N, w, counts), 8))
+    cases.append(("ms_elementwise_max", lambda: ms.ms_elementwise_max(N, w, w2, obs), 8 * 3))
+    xr = buf(3 * n - 2, N)
+    ms.ms_fill_uniforms(N, 3 * n - 2, ms.rng(1, 0, 0), xr, N)
+    cases.append(("ms_chili n=4 rows", lambda: ms.ms_chili(N, n, 13000.0 ** 2, None, [20.0] * n, None, xr, ms.rng(0), p, w, None, N),
+                  8 * (3 * n - 2 + 4 * (n + 2) + 1)))
+    out = []
+    for name, call, bytes_per_event in cases:
+        for _ in range(warmup):
+            call()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(steps):
+            call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        ms_call = ev[0].elapsed_time(ev[1]) / steps
+        row = {"case": name, "ms": ms_call, "alg_bytes_per_event": bytes_per_event,
+               "achieved_gbs": bytes_per_event * N / ms_call / 1e6}
+        if hbm_gbs > 0:
+            row["frac_of_hbm"] = row["achieved_gbs"] / hbm_gbs
+        out.append(row)
+    return {"probe": "next-rows", "events": N, "steps": steps, "results": out}
+
+
 def _hbm_peak() -> float:
     pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk):
@@ -390,6 +442,8 @@ def main() -> int:
         res = vegas_map(torch, hbm_gbs=_hbm_peak())
     elif what == "entry-points":
         res = entry_points(torch, hbm_gbs=_hbm_peak())
+    elif what == "next-rows":
+        res = next_rows(torch, hbm_gbs=_hbm_peak())
     else:
         raise SystemExit("unknown probe: " + what)
     print(json.dumps(res))
