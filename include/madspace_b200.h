@@ -66,7 +66,8 @@ typedef struct ms_rng {
 
 const char* ms_version(void);
 /* Raw cudaError_t of the last MS_ECUDA returned to the CALLING THREAD (thread-local; 0 if none). The library keeps no
- * other state: every call is re-entrant and may be issued from several host threads on different streams. */
+ * other state: every call is re-entrant and may be issued from several host threads on different streams -- with the one
+ * exception of ms_unweight_static, whose scratch is a device array shared by all its calls (see there). */
 int ms_last_cuda_error(void);
 
 /* Host-side validation of a VEGAS edge table h_edges[d][n_bins+1] (reading V-1):
