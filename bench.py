@@ -107,7 +107,7 @@ def alg_fp64_inverse(n: int) -> int:
     return c + 4 + RCP
 
 
-VEGAS_INVERSE_FP64_PER_VALUE = 8       # two subtractions, three-instruction quotient, j + q, / n_bins, one comparison
+VEGAS_INVERSE_FP64_PER_VALUE = 13      # x - x_j, five-instruction reciprocal refinement, three-instruction quotient, j + q, / n_bins, two comparisons
 PHILOX_IMAD_WIDE = 20                  # 32x32 -> 64-bit multiplies per Philox4x32-10 call (one per unweighting decision)
 
 
@@ -355,6 +355,14 @@ def stage_roofline(name, wl, N, t_ms, peaks, n_accepted=0, d_inv=0, traffic=None
         nbytes = N * 16 * d_inv
         sides = {"hbm": nbytes / hbm, "alu": N * d_inv * VEGAS_INVERSE_FP64_PER_VALUE / fp64}
         extra = {"alg_bytes_per_event": 16 * d_inv, "kernel": "ms::vegas_inverse_kernel"}
+    elif name == "inverse_fused":
+        # momenta -> uniforms in one kernel: the momenta read, the uniforms and the weight written; the x never reach HBM
+        nbytes = N * (32 * wl.n + 8 * d_inv + 8)
+        ninst = N * (alg_fp64_inverse(wl.n) + d_inv * VEGAS_INVERSE_FP64_PER_VALUE)
+        sides = {"hbm": nbytes / hbm, "alu": ninst / fp64}
+        extra = {"alg_bytes_per_event": 32 * wl.n + 8 * d_inv + 8,
+                 "alg_fp64_inst_per_event": alg_fp64_inverse(wl.n) + d_inv * VEGAS_INVERSE_FP64_PER_VALUE,
+                 "kernel": "ms::inverse_kernel<%d, grid>" % wl.n}
     else:
         return None
     bound = max(sides, key=sides.get)
@@ -500,6 +508,21 @@ def measure_config(torch, ms, name, steps, warmup, peaks, oracle_seconds):
     d_inv = 3 * wl.n - 4
     traffic = NCU_TRAFFIC.get(name, {})
     stages = {k: stage_roofline(k, wl, N, v, peaks, n_acc, d_inv, traffic.get(k)) for k, v in stage_ms.items()}
+    if "inverse_fused" in stage_ms:
+        # the two calls the fused inverse replaces are section 8(a) rows of their own (S9, S1 inverse): timed here too, on the
+        # same momenta, outside the step
+        for sname, fn in (("fastrambo_inverse", hp.invert_phase_space), ("vegas_inverse", hp.invert_grid)):
+            fn()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            torch.cuda.synchronize()
+            ev[0].record()
+            for _ in range(steps):
+                fn()
+            ev[1].record()
+            torch.cuda.synchronize()
+            st = stage_roofline(sname, wl, N, ev[0].elapsed_time(ev[1]) / steps, peaks, n_acc, d_inv, traffic.get(sname))
+            st["in_step"] = False
+            stages[sname] = st
     out = {"workload": "%s: %s" % (name, wl.note), "events_per_step": N, "steps": steps, "warmup": warmup,
            "ms_per_step": 1e3 * t_total / steps, "events_per_s": N * steps / t_total,
            "ms_per_step_median": float(np.median(per_step)), "stages": stages}

@@ -130,6 +130,18 @@ int ms_fastrambo(int64_t N, int n, double sqrt_s, const double* d_sqrt_s, const 
  * angles arbitrary), and the event's d_w is 0; a particle with zero momentum gets cos theta uniform 1/2, azimuth 0. */
 int ms_fastrambo_inverse(int64_t N, int n, const double* d_p, double* d_x, double* d_w, int64_t ld, void* stream);
 
+/* ms_fastrambo_inverse_vegas -- ms_fastrambo_inverse followed by the inverse direction of ms_vegas_map, in one kernel: the
+ * momenta are mapped straight to the uniforms r of a fused generation (Eq. 64, then :603), and the 3n-4
+ * phase-space variables never travel through HBM (the two calls write and re-read 16 B per variable and event).
+ *   d_edges: [grid_dims][grid_bins + 1], grid_dims == 3n-4 exactly, grid_bins 64 or 128 (the grids of the BASELINE.json
+ *            configs; any other grid: MS_EINVAL -- use the two calls).
+ *   d_r: [3n-4][ld] out.  Bit for bit what ms_vegas_map(direction 1) returns on the d_x of ms_fastrambo_inverse: same
+ *        search, same quotient.
+ *   d_w: [N] out or NULL: the weight of ms_fastrambo_inverse times the grid's Jacobian prod_j grid_bins * w_j, i.e. the
+ *        weight ms_generate returns for these uniforms (no PDF, no integrand). */
+int ms_fastrambo_inverse_vegas(int64_t N, int n, const double* d_p, const double* d_edges, int grid_dims, int grid_bins,
+                               double* d_r, double* d_w, int64_t ld, void* stream);
+
 /* ms_massive_rescale -- massive extension, strategy (i) of PAPER.md:510 (momentum rescaling of classic
  * RAMBO, ref. [64]; readings K-1..K-3): solve sum_i sqrt(m_i^2 + xi^2 E_i^2) = sqrt_s for xi by Newton
  * in registers (the first two steps are Halley's third-order variant of the Newton step, the rest plain Newton) until

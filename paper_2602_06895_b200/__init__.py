@@ -25,7 +25,7 @@ MS_UNWEIGHT_STATIC_MAX_EVENTS = 1 << 24
 
 EXPORTS = ("ms_version", "ms_last_cuda_error", "ms_check_grid", "ms_vegas_map", "ms_vegas_accumulate", "ms_vegas_refine", "ms_rambo_massless", "ms_fastrambo",
            "ms_fastrambo_inverse", "ms_massive_rescale", "ms_rambo_massive_reweight", "ms_rambo_massive_reweight_inverse", "ms_chili", "ms_pdf_x_boost", "ms_toy_integrand", "ms_reduce_max",
-           "ms_unweight_scratch_bytes", "ms_unweight", "ms_unweight_static", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_gather", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
+           "ms_unweight_scratch_bytes", "ms_unweight", "ms_unweight_static", "ms_fastrambo_inverse_vegas", "ms_weight_histogram", "ms_wmax_from_histogram", "ms_elementwise_max", "ms_gather", "ms_observable", "ms_cut", "ms_histogram_fill", "ms_invariant_map", "ms_generate", "ms_generate_unweight", "ms_unweight_compact", "ms_accept_bits_words", "ms_fill_uniforms")
 
 
 class MadSpaceError(RuntimeError):
@@ -88,6 +88,7 @@ def lib() -> C.CDLL:
         L.ms_toy_integrand.argtypes = [_i64, _int, _dbl, _vp, _vp, _int, _i64, _vp]
         L.ms_reduce_max.argtypes = [_i64, _vp, _vp, _vp]
         L.ms_unweight.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _i64, _vp]
+        L.ms_fastrambo_inverse_vegas.argtypes = [_i64, _int, _vp, _vp, _int, _int, _vp, _vp, _i64, _vp]
         L.ms_unweight_static.argtypes = [_i64, _vp, _vp, ms_rng, _int, _vp, _i64, _vp, _vp, _vp, _vp, _i64, _vp]
         L.ms_generate.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp]
         L.ms_generate_unweight.argtypes = [C.POINTER(ms_gen_config), _i64, ms_rng, _vp, _vp, _vp, _vp, _i64, _vp, _vp, ms_rng, _vp, _vp]
@@ -164,6 +165,11 @@ def ms_fastrambo(N, n, sqrt_s, d_sqrt_s, d_x, r: ms_rng, d_p, d_w, ld, d_fail=No
 
 def ms_fastrambo_inverse(N, n, d_p, d_x, d_w, ld, stream=None) -> None:
     _check("ms_fastrambo_inverse", lib().ms_fastrambo_inverse(N, n, _ptr(d_p), _ptr(d_x), _ptr(d_w), ld, _stream(stream)))
+
+
+def ms_fastrambo_inverse_vegas(N, n, d_p, d_edges, grid_dims, grid_bins, d_r, d_w, ld, stream=None) -> None:
+    _check("ms_fastrambo_inverse_vegas", lib().ms_fastrambo_inverse_vegas(N, n, _ptr(d_p), _ptr(d_edges), grid_dims, grid_bins,
+                                                                          _ptr(d_r), _ptr(d_w), ld, _stream(stream)))
 
 
 def ms_massive_rescale(N, n, sqrt_s, masses: Sequence[float], rel_tol, max_iter, d_p, d_w, ld, d_fail=None,

@@ -74,7 +74,17 @@ cudaError_t MS_CAT(launch_gen_exact_, MS_N)
 #else
 cudaError_t MS_CAT(launch_inverse_, MS_N)(const InvParams& P, bool massive, cudaStream_t stream)
 {
-    if (massive) {
+    if (P.edges != nullptr) {                               // straight through the inverse of a 64- or 128-bin grid
+        if (massive || MS_N < 2 || (P.grid_bins != 64 && P.grid_bins != 128)) return cudaErrorInvalidValue;
+        const int levels = P.grid_bins == 64 ? 6 : 7;
+        const size_t smem = vinv_table_bytes(3 * MS_N - 4, P.grid_bins, levels);
+        auto kernel = levels == 6 ? inverse_kernel<MS_N, false, 6> : inverse_kernel<MS_N, false, 7>;
+        if (smem > 48 * 1024) {
+            const cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (err != cudaSuccess) return err;
+        }
+        kernel<<<grid_for(kernel, P.N, smem), kBlock, smem, stream>>>(P);
+    } else if (massive) {
         auto kernel = inverse_kernel<MS_N, true>;
         kernel<<<grid_for(kernel, P.N, 0), kBlock, 0, stream>>>(P);
     } else {

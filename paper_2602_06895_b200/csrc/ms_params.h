@@ -66,6 +66,9 @@ struct InvParams {
     double* x;
     double* w;                 // or nullptr
     double phi_unit;
+    const double* edges;       // ms_fastrambo_inverse_vegas: [3n-4][grid_bins + 1], else nullptr (x = the phase-space variables)
+    int grid_bins;             // 64 or 128
+    double jac_scale;          // grid_bins^(3n-4)
     double masses[kMaxN];      // massive inverse only
     double msuf[kMaxN + 1];    // msuf[i] = sum_{j >= i} masses[j]
 };

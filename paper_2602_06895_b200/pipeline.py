@@ -4,7 +4,7 @@ tests check).  Marshalling and buffer ownership only: every arithmetic step is a
 One step = ms_generate (Philox -> VEGAS -> [x1,x2] -> Rambo/FastRambo -> [rescale] -> [boost] -> [toy] -> weight)
            [unweighting: ms_generate_unweight instead -- the hit-or-miss decision against w_max of the pre-run (computed
             once per grid) is taken in the generation kernel -- then ms_unweight_compact (stable compaction)]
-           [-> ms_fastrambo_inverse -> ms_vegas_map(inverse)]            (round trip, cfg 5)
+           [-> ms_fastrambo_inverse_vegas, or ms_fastrambo_inverse -> ms_vegas_map(inverse)]   (round trip, cfg 5)
 """
 from __future__ import annotations
 
@@ -18,7 +18,7 @@ import torch
 from . import (ms_elementwise_max, ms_weight_histogram, ms_wmax_from_histogram, MS_HIST_BINS,
                ms_vegas_accumulate, ms_vegas_refine, gen_config, ms_check_grid, ms_fastrambo_inverse, ms_generate, ms_reduce_max, ms_unweight,
                ms_unweight_scratch_bytes, ms_vegas_map, rng, MadSpaceError, MS_EGRID, ms_generate_unweight,
-               ms_unweight_compact, ms_accept_bits_words, ms_gather)
+               ms_unweight_compact, ms_accept_bits_words, ms_gather, ms_fastrambo_inverse_vegas)
 
 
 @contextlib.contextmanager
@@ -66,7 +66,7 @@ class PathSpec:
 
 class HotPath:
     def __init__(self, spec: PathSpec, N: int, device="cuda:0", cap: Optional[int] = None, gather_rows: bool = True,
-                 fuse_decision: bool = True):
+                 fuse_decision: bool = True, fuse_inverse: bool = True):
         if not torch.cuda.is_available():
             raise RuntimeError("HotPath needs a CUDA device: there is no CPU fallback")
         self.spec, self.N, self.device = spec, int(N), torch.device(device)
@@ -102,6 +102,9 @@ class HotPath:
             self.fuse_decision = bool(fuse_decision)
             self.accept_bits = torch.empty(max(ms_accept_bits_words(self.N), 4), dtype=torch.int32, device=self.device)
             self._bits_offset = None                           # event offset the bits in accept_bits belong to
+        # fuse_inverse: the round trip goes momenta -> uniforms in one kernel where ms_fastrambo_inverse_vegas applies
+        # (can_fuse_inverse); False keeps ms_fastrambo_inverse + ms_vegas_map (same r_inv, bit for bit)
+        self.fuse_inverse = bool(fuse_inverse)
         if spec.inverse:
             self.d_inv = 3 * spec.n - 4
             self.x_inv = torch.empty((self.d_inv, self.ld), **f64)
@@ -207,7 +210,24 @@ class HotPath:
                 ms_vegas_map(self.N, self.d_inv, self.grid_bins, self.d_edges, 1, self.x_inv, rng(0), self.r_inv, None,
                              self.ld, None)
 
+    @property
+    def can_fuse_inverse(self) -> bool:
+        """ms_fastrambo_inverse_vegas serves the round trip: a 64- or 128-bin grid of exactly 3n-4 dimensions on the
+        massless FastRambo chain."""
+        s = self.spec
+        return (self.d_edges is not None and self.grid_dims == 3 * s.n - 4 and self.grid_bins in (64, 128)
+                and s.mapping == "fastrambo" and not s.masses and not s.pdf)
+
+    def invert_fused(self, stream=None) -> None:
+        """Momenta -> uniforms in one kernel (r_inv, w_inv = weight with the grid's Jacobian); x_inv is not written."""
+        with _on(stream):
+            ms_fastrambo_inverse_vegas(self.N, self.spec.n, self.p, self.d_edges, self.grid_dims, self.grid_bins, self.r_inv,
+                                       self.w_inv, self.ld, None)
+
     def invert(self, stream=None) -> None:
+        if self.fuse_inverse and self.can_fuse_inverse:
+            self.invert_fused(stream)
+            return
         self.invert_phase_space(stream)
         self.invert_grid(stream)
 
@@ -226,9 +246,12 @@ class HotPath:
         if self.spec.unweight:
             out.append(("unweight", lambda off: self.unweight(off)))
         if self.spec.inverse:
-            out.append(("fastrambo_inverse", lambda off: self.invert_phase_space()))
-            if self.d_edges is not None:
-                out.append(("vegas_inverse", lambda off: self.invert_grid()))
+            if self.fuse_inverse and self.can_fuse_inverse:
+                out.append(("inverse_fused", lambda off: self.invert_fused()))
+            else:
+                out.append(("fastrambo_inverse", lambda off: self.invert_phase_space()))
+                if self.d_edges is not None:
+                    out.append(("vegas_inverse", lambda off: self.invert_grid()))
         return out
 
     def capture(self, event_offset: int = 0) -> "torch.cuda.CUDAGraph":
@@ -252,7 +275,7 @@ class HotPath:
         if self.spec.unweight:
             k += 2                                  # count (or decide) / scatter
         if self.spec.inverse:
-            k += 2 if self.d_edges is not None else 1
+            k += 1 if (self.fuse_inverse and self.can_fuse_inverse) or self.d_edges is None else 2
         return k
 
     @property

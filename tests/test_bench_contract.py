@@ -121,7 +121,7 @@ def test_per_config_block_covers_every_config_and_stage():
             assert k in c, (name, k)
         assert c["bound"] in ("hbm", "alu") and 0 < c["frac"] < 1.1
         want = {"generate"} | ({"unweight"} if name in ("cfg2", "cfg5") else set()) \
-            | ({"fastrambo_inverse", "vegas_inverse"} if name == "cfg5" else set())
+            | ({"inverse_fused", "fastrambo_inverse", "vegas_inverse"} if name == "cfg5" else set())
         assert set(c["stages"]) == want, (name, set(c["stages"]))
         for sname, st in c["stages"].items():
             for k in STAGE_KEYS:

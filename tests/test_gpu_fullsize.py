@@ -42,7 +42,9 @@ def test_full_size_step(ms, orc, name):
     from paper_2602_06895_b200.pipeline import HotPath
     wl = ms_inputs.WORKLOADS[name]
     N, n = wl.N, wl.n
-    hp = HotPath(path_spec(wl), N, DEV, cap=max(1 << 16, N // 256))      # bench.py's configuration
+    # bench.py's configuration, except that the round trip (cfg 5) runs as the two calls ms_fastrambo_inverse + ms_vegas_map, whose
+    # x-space output and phase-space weight are checked below; the fused call is then compared with them bit for bit
+    hp = HotPath(path_spec(wl), N, DEV, cap=max(1 << 16, N // 256), fuse_inverse=False)
     hp.step(0)
     torch.cuda.synchronize()
     assert int(hp.fail.item()) == 0
@@ -148,3 +150,17 @@ def test_full_size_step(ms, orc, name):
         print("inverse weight vs forward weight: max rel = %.3e, max rel/bound = %.3g, beyond 1e-12: %d of %d"
               % (rel_ps.max(), (rel_ps / bound).max(), int((rel_ps > 1e-12).sum()), rel_ps.size))
         assert np.all(rel_ps <= bound) and np.median(rel_ps) <= 1e-13
+        # the fused inverse (bench.py's default): the same uniforms bit for bit over all 20 x 2^24 values, and the phase-space
+        # weight times the grid's Jacobian
+        assert hp.can_fuse_inverse
+        r_two = hp.r_inv.clone()
+        w_two = hp.w_inv.clone()
+        hp.r_inv.zero_()
+        hp.invert_fused()
+        torch.cuda.synchronize()
+        assert torch.equal(hp.r_inv[:, :N], r_two[:, :N])
+        jac = (nb * width).prod(dim=0)                                    # of the generating bins = the bins found (r' ~ r)
+        ok = dr.amax(dim=0) < 0.25 / nb                                   # events whose r' stayed in r's bins
+        rel_j = ((hp.w_inv[:N] - w_two[:N] * jac).abs() / (w_two[:N] * jac))[ok]
+        assert int(ok.sum()) > 0.999 * N and float(rel_j.max()) <= 1e-12
+        del r_two, w_two
