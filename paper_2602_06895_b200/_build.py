@@ -19,7 +19,7 @@ LIB = os.path.join(_HERE, "libmadspace_b200.so")
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-diag-suppress", "177"]
-HEADERS = ["ms_math.cuh", "ms_kernels.cuh", "ms_params.h", "ms_launch.h"]
+HEADERS = ["ms_math.cuh", "ms_kernels.cuh", "ms_params.h", "ms_launch.h", "ms_vegas_inv.cuh"]
 N_RANGE = range(9, 1, -1)
 
 
