@@ -95,6 +95,25 @@ def test_host_side_argument_errors(ms):
     assert _code(ms, ms.ms_fastrambo, 8, 4, 1000.0, None, None, bad, FAKE, FAKE, 8, None, 0) == ms.MS_EINVAL
 
 
+def test_round_2_entry_points_validate_on_the_host(ms):
+    """ms_fastrambo_inverse_vegas and ms_unweight_static reject bad sizes before any CUDA call (no GPU needed)."""
+    r1 = ms.rng(3, 1)
+    # the grid must have exactly 3n-4 dimensions and 64 or 128 bins
+    for gd, gb in ((7, 128), (9, 128), (8, 100), (8, 256), (8, 32)):
+        assert _code(ms, ms.ms_fastrambo_inverse_vegas, 8, 4, FAKE, FAKE, gd, gb, FAKE, None, 8, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_fastrambo_inverse_vegas, 8, 4, FAKE, None, 8, 128, FAKE, None, 8, 0) == ms.MS_EINVAL
+    assert _code(ms, ms.ms_fastrambo_inverse_vegas, 8, 4, FAKE, FAKE, 8, 128, FAKE, None, 7, 0) == ms.MS_EINVAL     # ld < N
+    assert _code(ms, ms.ms_fastrambo_inverse_vegas, (1 << 31) + 1, 4, FAKE, FAKE, 8, 128, FAKE, None, (1 << 31) + 2, 0) == ms.MS_EINVAL
+    # beyond the static scratch: MS_ELIMIT, a code of its own
+    big = ms.MS_UNWEIGHT_STATIC_MAX_EVENTS + 1
+    assert _code(ms, ms.ms_unweight_static, big, FAKE, FAKE, r1, 0, None, 16, FAKE, FAKE, None, FAKE, big, 0) == ms.MS_ELIMIT
+    assert ms.MS_ELIMIT == -5 and _code(ms, ms.ms_unweight_static, -1, FAKE, FAKE, r1, 0, None, 16, FAKE, FAKE, None, FAKE, 8, 0) == ms.MS_EINVAL
+    header = open(os.path.join(ROOT, "include", "madspace_b200.h")).read()
+    assert "#define MS_UNWEIGHT_STATIC_MAX_EVENTS ((int64_t)1 << 24)" in header and ms.MS_UNWEIGHT_STATIC_MAX_EVENTS == 1 << 24
+    # the scratch the static array provides is what ms_unweight asks for at the maximum size
+    assert ms.ms_unweight_scratch_bytes(1 << 24) == int(re.search(r"#define MS_UNWEIGHT_STATIC_SCRATCH_BYTES (\d+)", header).group(1))
+
+
 def test_batches_beyond_the_32_bit_event_index_are_rejected(ms):
     """The per-multiplicity kernels index events with 32 bits; N > MS_MAX_EVENTS = 2^31 returns MS_EINVAL before any
     launch instead of silently processing N mod 2^32 events."""
